@@ -1,0 +1,328 @@
+"""Pins of the CPU oracle's grid-side functions: areas (Eq.8), deposit (Eq.21-23), field
+update (Eq.9-11, B8-B11), sort/compaction -- against closed forms, library routines,
+brute force and the invariants the paper states."""
+import math
+
+import numpy as np
+import pytest
+import scipy.integrate
+
+import oracle
+from paper_2503_04558_b200 import inputs
+
+
+def small_params(nr=24, nth=20, a=0.9, **kw):
+    return inputs.grid_params(nr, nth, a, r_out=20.0, **kw)
+
+
+# ------------------------------------------------------------------ quadrature, areas
+def test_gauss_legendre_nodes():
+    x, w = oracle.gauss_legendre(10)
+    xr, wr = np.polynomial.legendre.leggauss(10)
+    o = np.argsort(x)
+    assert np.allclose(x[o], xr, atol=1e-15) and np.allclose(w[o], wr, atol=1e-15)
+
+
+def test_areas_against_scipy_quad_and_closed_form():
+    p = small_params(12, 10, 0.95)
+    g = oracle.Grid(p)
+    A = oracle.areas(p)
+    a, dxi, dth, dphi = p["a"], g.dxi, g.dth, p["dphi"]
+    sg = lambda r, th: float(inputs.kerr_schild(a, 1.0, r, th)["sqrtg"])
+    r_ = lambda i: math.exp(p["xi_in"] + i * dxi)
+    for (i, j) in [(0, 0), (3, 4), (11, 10), (5, 9), (-1, 3)]:
+        tlo, thi = max((j - .5) * dth, 0), min((j + .5) * dth, math.pi)
+        ref = dphi * scipy.integrate.quad(lambda t: sg(r_(i + .5), t), tlo, thi, epsabs=0, epsrel=1e-13)[0]
+        assert np.isclose(A["ADr"][g.ij(i, j)], ref, rtol=1e-12)
+        ref = dphi * scipy.integrate.quad(lambda r: sg(r, j * dth), r_(i), r_(i + 1), epsabs=0, epsrel=1e-13)[0]
+        assert np.isclose(A["ABth"][g.ij(i, j)], ref, rtol=1e-12, atol=1e-16)
+        ref = scipy.integrate.dblquad(lambda t, r: sg(r, t), r_(i - .5), r_(i + .5), tlo, thi,
+                                      epsabs=0, epsrel=1e-12)[0]
+        assert np.isclose(A["ADph"][g.ij(i, j)], ref, rtol=1e-11)
+        if j < p["nth"]:
+            ref = dphi * scipy.integrate.quad(lambda r: sg(r, (j + .5) * dth), r_(i - .5), r_(i + .5), epsabs=0, epsrel=1e-13)[0]
+            assert np.isclose(A["ADth"][g.ij(i, j)], ref, rtol=1e-12)
+            ref = dphi * scipy.integrate.quad(lambda t: sg(r_(i), t), j * dth, (j + 1) * dth, epsabs=0, epsrel=1e-13)[0]
+            assert np.isclose(A["ABr"][g.ij(i, j)], ref, rtol=1e-12)
+            ref = scipy.integrate.dblquad(lambda t, r: sg(r, t), r_(i), r_(i + 1), j * dth, (j + 1) * dth,
+                                          epsabs=0, epsrel=1e-12)[0]
+            assert np.isclose(A["ABph"][g.ij(i, j)], ref, rtol=1e-11)
+    # a = 0 closed form: A^B_r = dphi r^2 sqrt(1+2/r) (cos th_j - cos th_{j+1})
+    p0 = small_params(12, 10, 0.0)
+    g0, A0 = oracle.Grid(p0), oracle.areas(p0)
+    i, j = 4, 3
+    r = math.exp(p0["xi_in"] + i * g0.dxi)
+    ref = p0["dphi"] * r * r * math.sqrt(1 + 2 / r) * (math.cos(j * g0.dth) - math.cos((j + 1) * g0.dth))
+    assert np.isclose(A0["ABr"][g0.ij(i, j)], ref, rtol=1e-13)
+    # total volume of the a=0 shell = dphi * int r^2 sqrt(1+2/r) dr * 2
+    tot = sum(A0["ABph"][g0.ij(i, j)] for i in range(p0["nr"]) for j in range(p0["nth"]))
+    ref = 2 * scipy.integrate.quad(lambda r: r * r * math.sqrt(1 + 2 / r), math.exp(p0["xi_in"]), 20.0, epsabs=0, epsrel=1e-13)[0]
+    assert np.isclose(tot, ref, rtol=1e-12)
+
+
+# ------------------------------------------------------------------ deposit
+def random_moves(p, n, seed, maxmove=0.9, axis_crossers=True):
+    rng = np.random.default_rng(seed)
+    g = oracle.Grid(p)
+    x = rng.uniform(0, p["nr"], n)
+    y = rng.uniform(0, p["nth"], n)
+    if axis_crossers:
+        y[: n // 5] = rng.uniform(0, 0.4, n // 5)
+        y[n // 5: 2 * n // 5] = p["nth"] - rng.uniform(0, 0.4, n // 5)
+    xn = x + rng.uniform(-maxmove, maxmove, n)
+    yn = y + rng.uniform(-maxmove, maxmove, n)
+    old = dict(x1=p["xi_in"] + x * g.dxi, x2=y * g.dth, x3=rng.uniform(0, 6, n),
+               flag=rng.integers(0, 2, n).astype(np.uint32))
+    new = dict(x1=p["xi_in"] + xn * g.dxi, x2dep=yn * g.dth, x3=old["x3"] + rng.uniform(-.1, .1, n))
+    # reflected new position (what the pusher stores)
+    x2 = new["x2dep"].copy()
+    x2 = np.where(x2 < 0, -x2, x2)
+    x2 = np.where(x2 > np.pi, 2 * np.pi - x2, x2)
+    new["x2"] = x2
+    new["flag"] = old["flag"].copy()
+    w = rng.uniform(0.5, 2.0, n)
+    return old, new, w
+
+
+def test_deposit_continuity_to_roundoff():
+    """Eq.(21): d(rho dV)/dt + div(F) = 0 node by node, incl. the axis nodes (fold)."""
+    p = small_params()
+    g = oracle.Grid(p)
+    old, new, w = random_moves(p, 400, 1)
+    dt = 0.013
+    F = oracle.fold_current(p, oracle.deposit(p, old, new, w, dt))
+    rho0 = oracle.rho(p, old, w, divide=False)
+    rho1 = oracle.rho(p, new, w, divide=False)
+    G = g.G
+    Fr, Fth = F[0], F[1]
+    # interior nodes i = 1..nr-1 (radial edge nodes exchange charge with the guards), all j = 0..nth
+    res = (rho1 - rho0) / dt
+    div = np.zeros_like(res)
+    div[G:G + p["nth"] + 1, 1:] += Fr[G:G + p["nth"] + 1, 1:] - Fr[G:G + p["nth"] + 1, :-1]
+    div[G:G + p["nth"] + 1, :] += Fth[G:G + p["nth"] + 1, :] - Fth[G - 1:G + p["nth"], :]
+    tot = (res + div)[G:G + p["nth"] + 1, G + 1:G + p["nr"]]
+    scale = np.max(np.abs(rho1)) / dt
+    assert np.max(np.abs(tot)) <= 1e-13 * scale, np.max(np.abs(tot)) / scale
+    assert np.max(np.abs(res)) > 1e-3 * scale         # non-trivial
+
+
+def test_deposit_bruteforce_whole_row_prefix_sum():
+    """Literal Eq.(21)-(22): W_r, W_th on EVERY node of the (padded) grid, prefix sums along
+    whole rows/columns; Eq.(23) on every node.  1..8 particles."""
+    p = small_params(10, 8, 0.7)
+    g = oracle.Grid(p)
+    G, dt = g.G, 0.02
+    for n in (1, 2, 5, 8):
+        old, new, w = random_moves(p, n, 10 + n)
+        F = oracle.deposit(p, old, new, w, dt)
+        I = np.arange(-G, p["nr"] + G + 1)[None, :]
+        J = np.arange(-G, p["nth"] + G + 1)[:, None]
+        S = lambda x, y: np.maximum(0, 1 - np.abs(x - I)) * np.maximum(0, 1 - np.abs(y - J))
+        Fr = np.zeros(g.shape); Fth = np.zeros(g.shape); Fph = np.zeros(g.shape)
+        for k in range(n):
+            Q = (1.0 if old["flag"][k] & 1 else -1.0) * w[k]
+            xa, xb = (old["x1"][k] - p["xi_in"]) / g.dxi, (new["x1"][k] - p["xi_in"]) / g.dxi
+            ya, yb = old["x2"][k] / g.dth, new["x2dep"][k] / g.dth
+            Wr = 0.5 * Q * (S(xb, yb) - S(xa, yb) + S(xb, ya) - S(xa, ya))
+            Wth = 0.5 * Q * (S(xb, yb) - S(xb, ya) + S(xa, yb) - S(xa, ya))
+            Fr += -np.cumsum(Wr, axis=1) / dt
+            Fth += -np.cumsum(Wth, axis=0) / dt
+            Fph += Q * (new["x3"][k] - old["x3"][k]) / dt * (S(xb, yb) / 3 + S(xb, ya) / 6 + S(xa, yb) / 6 + S(xa, ya) / 3)
+        sc = max(np.max(np.abs(Fr)), np.max(np.abs(Fth)))
+        assert np.max(np.abs(F[0] - Fr)) < 1e-13 * sc
+        assert np.max(np.abs(F[1] - Fth)) < 1e-13 * sc
+        assert np.max(np.abs(F[2] - Fph)) < 1e-13 * np.max(np.abs(Fph))
+
+
+def test_deposit_moments_and_sign():
+    """sum F_ph = sum Q dphi/dt; sum F_r = sum Q (x'-x)/dt in index units: a positive charge
+    moving to larger r gives positive J^r (sign convention of Eq.4 / reading G5)."""
+    p = small_params()
+    g = oracle.Grid(p)
+    old, new, w = random_moves(p, 300, 5, axis_crossers=False)
+    dt = 0.01
+    F = oracle.deposit(p, old, new, w, dt)
+    Q = np.where(old["flag"] & 1, 1.0, -1.0) * w
+    assert np.isclose(F[2].sum(), np.sum(Q * (new["x3"] - old["x3"])) / dt, rtol=1e-12)
+    assert np.isclose(F[0].sum(), np.sum(Q * (new["x1"] - old["x1"]) / g.dxi) / dt, rtol=1e-11)
+    assert np.isclose(F[1].sum(), np.sum(Q * (new["x2dep"] - old["x2"]) / g.dth) / dt, rtol=1e-11)
+
+
+def test_rho_total_charge():
+    p = small_params()
+    old, _, w = random_moves(p, 200, 7)
+    Q = np.where(old["flag"] & 1, 1.0, -1.0) * w
+    assert np.isclose(oracle.rho(p, old, w, divide=False).sum(), Q.sum(), rtol=1e-12)
+
+
+# ------------------------------------------------------------------ field solver
+def interior(g, X, m=2):
+    return X[g.G + m:g.G + g.nth + 1 - m, g.G + m:g.G + g.nr + 1 - m]
+
+
+@pytest.mark.parametrize("kind", ["wald", "monopole"])
+def test_analytic_solutions_are_discretely_stationary_second_order(kind):
+    """Appendix C fields are exact stationary vacuum solutions, so the discrete circulations
+    (B8)-(B11) vanish as Delta^2.  Fails O(1) without the 1/2 in E_phi (reading G2) or with a
+    wrong sign / index offset anywhere in B8-B11."""
+    res = []
+    for n in (16, 32, 64):
+        p = inputs.grid_params(n, n, 0.9, r_out=20.0, r_in=1.3)
+        g = oracle.Grid(p)
+        f = inputs.analytic_fields(p, kind)
+        Cs = oracle.circulation(p, f)
+        # fixed physical sub-domain (1/8 of the range away from every boundary and the axis)
+        res.append([np.max(np.abs(interior(g, Cs[c], n // 8))) for c in range(6)])
+    res = np.array(res)
+    assert np.all(res[2] < 2e-3), res[2]
+    for c in range(6):
+        if res[0, c] > 1e-9:
+            assert res[0, c] / res[1, c] > 2.5 and res[1, c] / res[2, c] > 3.3, (c, res[:, c])
+
+
+def divB(g, A, f):
+    G, nr, nth = g.G, g.nr, g.nth
+    Br, Bth = f[3] * A["ABr"], f[4] * A["ABth"]
+    # cell (i+1/2, j+1/2), i<nr, j<nth
+    return (Br[G:G + nth, G + 1:G + nr + 1] - Br[G:G + nth, G:G + nr]) + \
+           (Bth[G + 1:G + nth + 1, G:G + nr] - Bth[G:G + nth, G:G + nr])
+
+
+def test_divB_preserved_exactly_and_linearity():
+    p = small_params(20, 16, 0.95, damp_cells=0)
+    g = oracle.Grid(p)
+    A = oracle.areas(p)
+    rng = np.random.default_rng(2)
+    f = [rng.normal(size=g.shape) for _ in range(6)]
+    f = oracle.apply_bc(p, f)
+    d0 = divB(g, A, f)
+    f1 = [x.copy() for x in f]
+    oracle.field_step(p, f1, None, 0.01)
+    d1 = divB(g, A, f1)
+    sc = np.max(np.abs(f[3] * A["ABr"]))
+    assert np.max(np.abs(d1 - d0)) < 1e-13 * sc
+    # linearity of the whole step in (D,B,J)
+    h = [rng.normal(size=g.shape) for _ in range(6)]
+    h = oracle.apply_bc(p, h)
+    J = [rng.normal(size=g.shape) for _ in range(3)]
+    s1 = oracle.field_step(p, [x.copy() for x in f], J, 0.01)
+    s2 = oracle.field_step(p, [x.copy() for x in h], None, 0.01)
+    s12 = oracle.field_step(p, [x + 2 * y for x, y in zip(f, h)], J, 0.01)
+    for c in range(6):
+        assert np.allclose(s12[c], s1[c] + 2 * s2[c], atol=1e-11 * np.max(np.abs(s12[c])))
+
+
+def test_field_step_heun_limit_and_euler():
+    """N=0 is forward Euler D^n + dt (C_H - J); N=1 with beta=1/2 is Heun's method
+    (reading G3)."""
+    p = small_params(16, 12, 0.9)
+    g = oracle.Grid(p)
+    f0 = inputs.analytic_fields(p, "wald")
+    f0[5] = f0[5] + 1e-2 * np.exp(-((np.arange(g.shape[1])[None, :] - 10.0) ** 2 + (np.arange(g.shape[0])[:, None] - 8.0) ** 2) / 8.0)
+    f0 = oracle.apply_bc(p, f0)
+    rng = np.random.default_rng(4)
+    J = [1e-3 * rng.normal(size=g.shape) for _ in range(3)]
+    dt = 0.004
+    # physical range of component c; D^ph, B^th are imposed (= 0) on the axis rows, skip those
+    ph = lambda X, c: X[g.G + (1 if c in (2, 4) else 0):g.G + g.nth + (0 if c in (1, 2, 3, 4, 5) else 1),
+                        g.G:g.G + g.nr + (0 if c in (0, 4, 5) else 1)]
+    # Euler
+    pe = dict(p, field_iters=0)
+    fe = oracle.field_step(pe, [x.copy() for x in f0], J, dt)
+    C0 = oracle.circulation(p, f0)
+    for c in range(6):
+        ref = f0[c] + dt * (C0[c] - (J[c] if c < 3 else 0))
+        assert np.allclose(ph(fe[c], c), ph(ref, c), atol=1e-14 * np.max(np.abs(ref)) + 1e-18), c
+    # Heun
+    phn = dict(p, field_iters=1, beta_impl=0.5)
+    fh = oracle.field_step(phn, [x.copy() for x in f0], J, dt)
+    C1 = oracle.circulation(p, oracle.apply_bc(p, [x.copy() for x in fe]))
+    for c in range(6):
+        ref = f0[c] + dt * (0.5 * C0[c] + 0.5 * C1[c] - (J[c] if c < 3 else 0))
+        assert np.allclose(ph(fh[c], c), ph(ref, c), atol=1e-14 * np.max(np.abs(ref)) + 1e-18), c
+
+
+def test_field_step_second_order_in_dt():
+    p = small_params(16, 12, 0.9, field_iters=7, beta_impl=0.5)
+    g = oracle.Grid(p)
+    f0 = inputs.analytic_fields(p, "monopole")
+    bump = 1e-2 * np.exp(-((np.arange(g.shape[1])[None, :] - 10.0) ** 2 + (np.arange(g.shape[0])[:, None] - 8.0) ** 2) / 8.0)
+    f0[5] = f0[5] + bump
+    f0 = oracle.apply_bc(p, f0)
+    T = 0.08
+    def run(n):
+        f = [x.copy() for x in f0]
+        for _ in range(n):
+            oracle.field_step(p, f, None, T / n)
+        return f
+    f1, f2, f4 = run(4), run(8), run(16)
+    e1 = max(np.max(np.abs(interior(g, a - b))) for a, b in zip(f1, f2))
+    e2 = max(np.max(np.abs(interior(g, a - b))) for a, b in zip(f2, f4))
+    assert 3.2 < e1 / e2 < 4.8, (e1, e2)
+
+
+def test_gauss_law_preserved_with_deposited_current():
+    """div D - rho is unchanged by a step when J comes from the charge-conserving deposit
+    (PAPER.md:130, :337), including the axis nodes (Eq.11)."""
+    p = small_params(20, 16, 0.9)
+    g = oracle.Grid(p)
+    A = oracle.areas(p)
+    dt = 0.01
+    old, new, w = random_moves(p, 300, 9, maxmove=0.45)
+    F = oracle.deposit(p, old, new, w, dt)
+    J = oracle.finalize_current(p, [x.copy() for x in F], 0)
+    f0 = oracle.apply_bc(p, inputs.analytic_fields(p, "monopole"))
+    f1 = oracle.field_step(p, [x.copy() for x in f0], J, dt)
+    G, nr, nth = g.G, g.nr, g.nth
+    def divD(f):
+        Dr, Dth = f[0] * A["ADr"], f[1] * A["ADth"]
+        d = np.zeros(g.shape)
+        d[:, 1:] += Dr[:, 1:] - Dr[:, :-1]
+        d[G + 1:G + nth, :] += Dth[G + 1:G + nth, :] - Dth[G:G + nth - 1, :]
+        d[G, :] += Dth[G, :]                     # axis theta=0: only the +1/2 face
+        d[G + nth, :] += -Dth[G + nth - 1, :]    # axis theta=pi
+        return d
+    drho = oracle.rho(p, new, w, divide=False) - oracle.rho(p, old, w, divide=False)
+    lhs = divD(f1) - divD(f0)
+    sel = (slice(G, G + nth + 1), slice(G + 1, G + nr))
+    sc = np.max(np.abs(drho))
+    assert np.max(np.abs((lhs - drho)[sel])) < 1e-12 * sc
+    assert sc > 0
+
+
+def test_damping_layer_profile():
+    p = small_params(20, 8, 0.9, damp_cells=5, damp_coef=0.8, field_iters=0)
+    g = oracle.Grid(p)
+    f = [np.ones(g.shape) for _ in range(6)]
+    bg = [np.full(g.shape, 0.25) for _ in range(6)]
+    out = oracle.field_step(p, [x.copy() for x in f], None, 0.0, bg=bg)
+    i0 = 15
+    for i in (14, 16, 18, 20):
+        s = max(0, i - i0) / 5
+        lam = 1 - 0.8 * s ** 3
+        assert np.isclose(out[2][g.ij(i, 3)], 0.25 + 0.75 * lam, rtol=1e-14)
+
+
+def test_filter_preserves_sums_and_kernel():
+    p = small_params(12, 10, 0.5)
+    g = oracle.Grid(p)
+    F = [np.zeros(g.shape) for _ in range(3)]
+    F[2][g.ij(5, 5)] = 16.0
+    ref_area = oracle.areas(p)
+    J = oracle.finalize_current(p, [x.copy() for x in F], 1)
+    back = J[2] * ref_area["ADph"] * p["dphi"]
+    assert np.isclose(back[g.ij(5, 5)], 4.0) and np.isclose(back[g.ij(4, 5)], 2.0)
+    assert np.isclose(back[g.ij(4, 4)], 1.0) and np.isclose(back.sum(), 16.0)
+
+
+# ------------------------------------------------------------------ sort / compaction
+def test_sort_and_compact_definitions():
+    rng = np.random.default_rng(0)
+    n = 5000
+    cell = rng.integers(0, 97, n).astype(np.uint32)
+    flag = (rng.integers(0, 2, n) | (2 * (rng.uniform(size=n) < 0.1))).astype(np.uint32)
+    perm = oracle.sort(cell, flag)
+    key = np.where(flag & 2, 0xFFFFFFFF, cell).astype(np.uint64)
+    assert np.array_equal(perm, np.argsort(key, kind="stable").astype(np.uint32))
+    idx = oracle.compact(flag)
+    assert np.array_equal(idx, np.nonzero((flag & 2) == 0)[0].astype(np.uint32))

@@ -1,0 +1,287 @@
+"""Pins of the CPU oracle's metric, geodesic integrator and Boris push against what the
+paper and the mathematics fix (not against the oracle itself, and never against CUDA)."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2503_04558_b200 import inputs
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def table1():
+    rows = {}
+    for line in open(os.path.join(HERE, "golden", "table1_orbits.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        t = line.split()
+        rows[t[0]] = dict(a=float(t[1]), B0=float(t[2]), ur=float(t[3]), uth=float(t[4]),
+                          uph=float(t[5]), r=float(t[6]), th=math.pi / 2 - float(t[7]))
+    return rows
+
+
+# ------------------------------------------------------------------ metric (Appendix A)
+@pytest.mark.parametrize("a,M,r,th", [(0.99, 1.0, 1.3, 0.4), (0.5, 1.0, 7.0, 2.5),
+                                      (0.0, 1.0, 3.0, 1.0), (0.9, 2.0, 5.0, 0.05)])
+def test_metric_inverse_det_and_sqrtg(a, M, r, th):
+    m = oracle.metric(a, M, r, th)
+    g = np.array([[m["g_rr"], 0, m["g_rph"]], [0, m["g_thth"], 0], [m["g_rph"], 0, m["g_phph"]]])
+    gu = np.array([[m["gu_rr"], 0, m["gu_rph"]], [0, m["gu_thth"], 0], [m["gu_rph"], 0, m["gu_phph"]]])
+    assert np.allclose(g @ gu, np.eye(3), atol=1e-13)
+    assert np.isclose(np.linalg.det(g), m["sqrtg"] ** 2, rtol=1e-13)
+    # 4-metric consistency: g_tt = beta^2 - alpha^2 = z - 1, g_tr = beta_r = z   (A2)
+    z = 2 * M * r / (r * r + a * a * math.cos(th) ** 2)
+    beta_lo_r = m["g_rr"] * m["beta_r"]
+    assert np.isclose(beta_lo_r * m["beta_r"] - m["alpha"] ** 2, z - 1.0, rtol=1e-13)
+    assert np.isclose(beta_lo_r, z, rtol=1e-13)
+    # g_t_phi = beta_phi = gamma_{phi r} beta^r = -a z sin^2     (A2)
+    assert np.isclose(m["g_rph"] * m["beta_r"], -a * z * math.sin(th) ** 2, rtol=1e-13, atol=1e-300)
+
+
+@pytest.mark.parametrize("a,M,r,th", [(0.99, 1.0, 1.3, 0.4), (0.5, 1.0, 7.0, 2.5), (0.9, 2.0, 5.0, 0.3)])
+def test_metric_derivatives_finite_difference(a, M, r, th):
+    m = oracle.metric(a, M, r, th)
+    h = 1e-5
+    for q in ("alpha", "beta", "gu_rr", "gu_thth", "gu_phph", "gu_rph"):
+        key = "beta_r" if q == "beta" else q
+        # 4th-order central differences
+        def f(rr, tt):
+            return oracle.metric(a, M, rr, tt)[key]
+        dr = (-f(r + 2 * h, th) + 8 * f(r + h, th) - 8 * f(r - h, th) + f(r - 2 * h, th)) / (12 * h)
+        dth = (-f(r, th + 2 * h) + 8 * f(r, th + h) - 8 * f(r, th - h) + f(r, th - 2 * h)) / (12 * h)
+        assert np.isclose(m["dr_" + q], dr, rtol=1e-8, atol=1e-10), q
+        assert np.isclose(m["dth_" + q], dth, rtol=1e-8, atol=1e-10), q
+
+
+def test_metric_matches_independent_form():
+    # the input generator writes Appendix A in a different algebraic form (no Sigma, Delta)
+    rng = np.random.default_rng(0)
+    for _ in range(20):
+        a, r, th = rng.uniform(0, 0.999), rng.uniform(1.0, 40.0), rng.uniform(0.01, 3.13)
+        m, k = oracle.metric(a, 1.0, r, th), inputs.kerr_schild(a, 1.0, r, th)
+        for key in ("alpha", "beta_r", "g_rr", "g_thth", "g_phph", "g_rph", "gu_rr", "gu_thth",
+                    "gu_phph", "gu_rph", "sqrtg"):
+            assert np.isclose(m[key], float(k[key]), rtol=1e-13), key
+
+
+# ------------------------------------------------------------------ geodesics
+def energy(a, M, y):
+    """E = -u_t = alpha^2 u^0 - beta^r u_r (massive)."""
+    m = oracle.metric(a, M, y[0], y[1])
+    u = y[3:6]
+    nrm = m["gu_rr"] * u[0] ** 2 + m["gu_thth"] * u[1] ** 2 + m["gu_phph"] * u[2] ** 2 + 2 * m["gu_rph"] * u[0] * u[2]
+    u0 = math.sqrt(1 + nrm) / m["alpha"]
+    return m["alpha"] ** 2 * u0 - m["beta_r"] * u[0]
+
+
+def test_geodesic_uphi_exact_and_energy_second_order():
+    o = table1()["(3,3,2)"]
+    y0 = np.array([o["r"], o["th"], 0.0, o["ur"], o["uth"], o["uph"]])
+    errs = []
+    for dt in (0.1, 0.05, 0.025):
+        n = int(round(120.0 / dt))
+        tr = oracle.geodesic_traj(o["a"], 1.0, 3, y0, dt, n, every=1)
+        assert np.all(tr[:, 5] == y0[5])           # U_phi = 0: bit-exact conservation
+        E = np.array([energy(o["a"], 1.0, y) for y in tr[:: max(1, n // 400)]])
+        errs.append(np.mean(np.abs(E - E[0])))
+    # "relative error decreases as dt^2"
+    assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
+
+
+@pytest.mark.parametrize("name,zwv", [("(2,0,1)", (2, 0, 1)), ("(3,3,1)", (3, 3, 1)),
+                                      ("(3,3,2)", (3, 3, 2)), ("(4,3,1)", (4, 3, 1))])
+def test_table1_periodic_orbit_taxonomy(name, zwv):
+    """Table 1 rows start at apoapsis; over one radial period the azimuth advances by
+    2 pi (1 + w + v/z) for a (z,w,v) periodic orbit."""
+    o = table1()[name]
+    z, w, v = zwv
+    y0 = np.array([o["r"], o["th"], 0.0, o["ur"], o["uth"], o["uph"]])
+    dt = 0.02
+    n = int(600.0 / dt)
+    tr = oracle.geodesic_traj(o["a"], 1.0, 3, y0, dt, n, every=1)
+    r, ph = tr[:, 0], tr[:, 2]
+    assert np.allclose(tr[:, 1], math.pi / 2, atol=1e-12)     # stays equatorial
+    # first interior local maximum of r after leaving apoapsis = next apoapsis
+    k = np.where((r[1:-1] > r[:-2]) & (r[1:-1] >= r[2:]) & (np.arange(1, n - 1) > 100))[0][0] + 1
+    # parabolic refinement of the apoapsis time
+    den = r[k - 1] - 2 * r[k] + r[k + 1]
+    off = 0.5 * (r[k - 1] - r[k + 1]) / den
+    phi_apo = ph[k] + off * 0.5 * (ph[k + 1] - ph[k - 1])
+    assert abs(phi_apo / (2 * math.pi) - (1 + w + v / z)) < 2e-3
+    assert abs(r[k] - o["r"]) < 2e-3 * o["r"]
+
+
+@pytest.mark.parametrize("a,rfac", [(0.0, 1.0), (0.9, 1.5), (0.99, 1.5)])
+def test_circular_orbit_frequency(a, rfac):
+    """Textbook prograde circular equatorial Kerr orbits (Bardeen, Press & Teukolsky 1972):
+    Omega = 1/(r^{3/2}+a); r_isco(a=0) = 6 gives Omega = 6^{-3/2} = 0.0680413817."""
+    Z1 = 1 + (1 - a * a) ** (1 / 3) * ((1 + a) ** (1 / 3) + (1 - a) ** (1 / 3))
+    Z2 = math.sqrt(3 * a * a + Z1 * Z1)
+    r_isco = 3 + Z2 - math.sqrt((3 - Z1) * (3 + Z1 + 2 * Z2))
+    if a == 0.0:
+        assert abs(r_isco - 6.0) < 1e-12
+    r = rfac * r_isco
+    den = r ** 0.75 * math.sqrt(r ** 1.5 - 3 * math.sqrt(r) + 2 * a)
+    E = (r ** 1.5 - 2 * math.sqrt(r) + a) / den
+    L = (r * r - 2 * a * math.sqrt(r) + a * a) / den
+    Delta = r * r + a * a - 2 * r
+    # BL -> KS covariant momentum (from A6): u_r^KS = u_r^BL + (2 r E - a L)/Delta
+    y0 = np.array([r, math.pi / 2, 0.0, (2 * r * E - a * L) / Delta, 0.0, L])
+    assert abs(energy(a, 1.0, y0) - E) < 1e-12
+    Omega = 1.0 / (r ** 1.5 + a)
+    T = 2 * math.pi / Omega
+    dt = T / 20000
+    tr = oracle.geodesic_traj(a, 1.0, 3, y0, dt, 20001, every=1)
+    assert np.max(np.abs(tr[:, 0] - r)) < 2e-6 * r
+    assert abs((tr[-1, 2] - tr[0, 2]) / (20000 * dt) - Omega) < 1e-7
+    if a == 0.0 and rfac == 1.0:
+        assert abs(Omega - 0.0680413817) < 1e-9
+
+
+def test_photon_null_and_energy():
+    a = 0.9
+    m = oracle.metric(a, 1.0, 6.0, 1.0)
+    y0 = np.array([6.0, 1.0, 0.0, 0.3, 1.0, 2.0])
+    tr = oracle.geodesic_traj(a, 1.0, 3, y0, 0.01, 2000, every=100, eps=0.0)
+    def Eph(y):
+        mm = oracle.metric(a, 1.0, y[0], y[1])
+        u = y[3:6]
+        nrm = mm["gu_rr"] * u[0] ** 2 + mm["gu_thth"] * u[1] ** 2 + mm["gu_phph"] * u[2] ** 2 + 2 * mm["gu_rph"] * u[0] * u[2]
+        return mm["alpha"] * math.sqrt(nrm) - mm["beta_r"] * u[0]
+    E = np.array([Eph(y) for y in tr])
+    assert np.max(np.abs(E - E[0])) < 1e-5 * abs(E[0])
+
+
+# ------------------------------------------------------------------ Boris (Eq.16-19)
+def _cross_lo(m, A, B):
+    return m["sqrtg"] * np.cross(A, B)
+
+
+def _raise(m, u):
+    return np.array([m["gu_rr"] * u[0] + m["gu_rph"] * u[2], m["gu_thth"] * u[1],
+                     m["gu_rph"] * u[0] + m["gu_phph"] * u[2]])
+
+
+def _lower(m, v):
+    return np.array([m["g_rr"] * v[0] + m["g_rph"] * v[2], m["g_thth"] * v[1],
+                     m["g_rph"] * v[0] + m["g_phph"] * v[2]])
+
+
+def test_boris_norm_residual_and_angle():
+    a, r, th = 0.99, 1.7, 0.6
+    m = oracle.metric(a, 1.0, r, th)
+    rng = np.random.default_rng(3)
+    u = rng.normal(size=3) * 3
+    B = rng.normal(size=3)
+    D = rng.normal(size=3) * 0.3
+    dt, sgn = 0.05, -1.0
+    # (i) pure magnetic rotation preserves gamma^ij u_i u_j to round-off
+    up = oracle.boris(a, 1.0, r, th, u, np.zeros(3), B, sgn, dt)
+    n0, n1 = u @ _raise(m, u), up @ _raise(m, up)
+    assert abs(n1 - n0) < 1e-13 * n0
+    # rotation angle = 2 atan sqrt(t_k t^k)
+    u0bar = math.sqrt(1 + n0) / m["alpha"]
+    t = sgn * B * dt / (2 * u0bar)
+    t2 = t @ _lower(m, t)
+    # decompose u^i perpendicular to B^i with the metric inner product
+    uu, upu = _raise(m, u), _raise(m, up)
+    Bl = _lower(m, B)
+    perp = lambda x: x - (x @ Bl) / (B @ Bl) * B
+    pa, pb = perp(uu), perp(upu)
+    cosang = (pa @ _lower(m, pb)) / math.sqrt((pa @ _lower(m, pa)) * (pb @ _lower(m, pb)))
+    assert abs(math.acos(cosang) - 2 * math.atan(math.sqrt(t2))) < 1e-12
+    # (ii) Eq.(16) with ubar = (u^- + u^+)/2 and ubar^0 of Eq.(18) is solved exactly
+    up = oracle.boris(a, 1.0, r, th, u, D, B, sgn, dt)
+    Dl = _lower(m, D)
+    um = u + sgn * m["alpha"] * dt / 2 * Dl
+    upl = up - sgn * m["alpha"] * dt / 2 * Dl
+    ubar = 0.5 * (um + upl)
+    u0b = math.sqrt(1 + um @ _raise(m, um)) / m["alpha"]
+    rhs = u + sgn * dt * (m["alpha"] * Dl + _cross_lo(m, _raise(m, ubar), B) / u0b)
+    assert np.max(np.abs(up - rhs)) < 1e-13 * np.max(np.abs(up))
+
+
+def test_flat_space_gyration():
+    """M = 0, a = 0: special-relativistic gyration in uniform B_z = B0:
+    B^r = B0 cos(th), B^th = -B0 sin(th)/r; |u| constant, phase advance per step
+    2 atan(q B0 dt / (2 m Gamma)); full push = Boris + straight-line geodesic."""
+    B0, dt = 2.0, 0.01
+    r, th, ph = 5.0, 1.1, 0.3
+    # Cartesian momentum (ux, uy, uz) -> covariant spherical components
+    ux, uy, uz = 1.5, -0.7, 0.4
+    Gam = math.sqrt(1 + ux * ux + uy * uy + uz * uz)
+    def to_cov(r, th, ph, ux, uy, uz):
+        er = np.array([math.sin(th) * math.cos(ph), math.sin(th) * math.sin(ph), math.cos(th)])
+        et = np.array([math.cos(th) * math.cos(ph), math.cos(th) * math.sin(ph), -math.sin(th)])
+        ep = np.array([-math.sin(ph), math.cos(ph), 0.0])
+        U = np.array([ux, uy, uz])
+        return np.array([U @ er, r * (U @ et), r * math.sin(th) * (U @ ep)]), (er, et, ep)
+    u, _ = to_cov(r, th, ph, ux, uy, uz)
+    pos = np.array([r * math.sin(th) * math.cos(ph), r * math.sin(th) * math.sin(ph), r * math.cos(th)])
+    y = np.array([r, th, ph, *u])
+    nsteps = 400
+    for _ in range(nsteps):
+        B = np.array([B0 * math.cos(y[1]), -B0 * math.sin(y[1]) / y[0], 0.0])
+        ub = oracle.boris(0.0, 0.0, y[0], y[1], y[3:6], np.zeros(3), B, +1.0, dt)
+        y = oracle.geodesic(0.0, 0.0, 3, np.array([y[0], y[1], y[2], *ub]), dt)
+    # back to Cartesian momentum
+    r1, th1, ph1 = y[0:3]
+    er = np.array([math.sin(th1) * math.cos(ph1), math.sin(th1) * math.sin(ph1), math.cos(th1)])
+    et = np.array([math.cos(th1) * math.cos(ph1), math.cos(th1) * math.sin(ph1), -math.sin(th1)])
+    ep = np.array([-math.sin(ph1), math.cos(ph1), 0.0])
+    U = y[3] * er + y[4] / r1 * et + y[5] / (r1 * math.sin(th1)) * ep
+    assert abs(np.linalg.norm(U) - math.sqrt(ux * ux + uy * uy + uz * uz)) < 1e-6
+    assert abs(U[2] - uz) < 1e-6                        # u_z unchanged along B
+    # positive charge in B_z gyrates clockwise: phase = -n * 2 atan(B0 dt/(2 Gamma)), up to the
+    # O(dt^2) splitting error of moving-frame bases
+    phase = math.atan2(U[1], U[0]) - math.atan2(uy, ux)
+    expect = -nsteps * 2 * math.atan(B0 * dt / (2 * Gam))
+    assert abs((phase - expect + math.pi) % (2 * math.pi) - math.pi) < 2e-4
+    # z advances uniformly
+    assert abs(r1 * math.cos(th1) - (pos[2] + uz / Gam * nsteps * dt)) < 1e-5
+
+
+# ------------------------------------------------------------------ charged orbit, Eq.(24)
+@pytest.mark.parametrize("name", ["RKA3", "RKA8"])
+def test_charged_orbit_conserves_eq24(name):
+    """Full step (Boris with the analytic Wald field of C14-C19 + geodesic) conserves
+    E = -u_0 - (q/m) A_0 (Eq.24) and L = u_phi + (q/m) A_phi, with the
+    potentials of (C12), to second order in dt."""
+    o = table1()[name]
+    a, B0, qm = o["a"], o["B0"], +1.0
+
+    def A_t(r, th):
+        c2 = math.cos(th) ** 2
+        return B0 * (a * r * (1 + c2) / (r * r + a * a * c2) - a)
+
+    def A_ph(r, th):
+        c2 = math.cos(th) ** 2
+        return B0 * 0.5 * math.sin(th) ** 2 * (r * r + a * a - 2 * a * a * r * (1 + c2) / (r * r + a * a * c2))
+
+    def half_boris(y, dt):
+        D = [float(v) for v in inputs.analytic_DB(a, 1.0, B0, y[0], y[1], "wald")]
+        ub = oracle.boris(a, 1.0, y[0], y[1], y[3:6], D[0:3], D[3:6], qm, 0.5 * dt)
+        return np.array([y[0], y[1], y[2], *ub])
+
+    def run(dt, T):
+        y = np.array([o["r"], o["th"], 0.0, o["ur"], o["uth"], o["uph"]])
+        E0 = energy(a, 1.0, y) - qm * A_t(y[0], y[1])
+        L0 = y[5] + qm * A_ph(y[0], y[1])
+        dE = dL = 0.0
+        for _ in range(int(round(T / dt))):
+            # Strang sequence of PAPER.md:155: half Boris, full geodesic, half Boris at the new
+            # position (the production loop bundles adjacent halves into one full Boris, :204)
+            y = half_boris(y, dt)
+            y = oracle.geodesic(a, 1.0, 3, y, dt)
+            y = half_boris(y, dt)
+            dE = max(dE, abs(energy(a, 1.0, y) - qm * A_t(y[0], y[1]) - E0))
+            dL = max(dL, abs(y[5] + qm * A_ph(y[0], y[1]) - L0))
+        return dE / abs(E0), dL / abs(L0)
+
+    e1, l1 = run(0.02, 20.0)
+    e2, l2 = run(0.01, 20.0)
+    assert e1 < 2e-3 and l1 < 2e-3
+    assert 2.8 < e1 / e2 < 5.5 and 2.8 < l1 / l2 < 5.5, (e1, e2, l1, l2)
