@@ -1,0 +1,157 @@
+/* grpic.h -- C ABI of libgrpic.so: the B200-native (sm_100a) data-parallel hot path of the
+ * GRPIC method of arxiv 2503.04558 (Aperture): general-relativistic particle push fused with
+ * charge-conserving current deposition on a 2D axisymmetric (log r, theta) Kerr-Schild Yee
+ * grid, the GR Maxwell (D,B) field update that consumes that current, and the particle
+ * cell-sort / compaction passes around them.
+ *
+ * Citations are to the paper text (PAPER.md:<line>, section / equation).
+ *
+ * Conventions
+ *  - Every array argument is a CALLER-OWNED DEVICE pointer (cudaMalloc / torch CUDA tensor)
+ *    unless it says "host".  The library never frees them and keeps no reference after the
+ *    call returns, except the workspace registered with grpic_set_workspace.
+ *  - All work is enqueued on the caller's CUDA stream (`void* stream` = cudaStream_t; NULL =
+ *    default stream) and is asynchronous; nothing synchronises the device.
+ *  - Every call returns 0 on success or a negative grpic error code for argument / state
+ *    errors found synchronously on the host (nothing is launched then).  Device-side
+ *    anomalies are OR-ed into a caller-provided device word `status` (see GRPIC_STATUS_*).
+ *  - No CPU fallback exists: without a CUDA device grpic_create fails with GRPIC_ERR_CUDA.
+ *
+ * Grid (Fig.1; Appendix B :476-518): nr x nth cells, nodes i=0..nr,
+ * j=0..nth, xi = ln r, xi_i = xi_in + i*dxi, theta_j = j*pi/nth.  Staggering, index (i,j) =
+ *     D^r, J^r, B^th : (i+1/2, j)     D^th, J^th, B^r : (i, j+1/2)
+ *     D^ph, J^ph, rho: (i, j)         B^ph            : (i+1/2, j+1/2)
+ * Every grid array has the same pitched layout, r fastest: element (i,j), i in [-ng, nr+ng],
+ * j in [-ng, nth+ng], lives at  (j + j0)*pitch + (i + i0)  with pitch, rows, i0, j0 from
+ * grpic_grid_layout (i = 0 is 32-byte aligned, pitch is a multiple of 16 doubles).
+ * Radial guard values are copies of the last physical value; theta ghost
+ * rows hold the parity image about the axis (r, phi components even, theta components odd).
+ */
+#ifndef GRPIC_H_
+#define GRPIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct grpic_ctx grpic_ctx; /* opaque; owns only its own metric/area tables */
+
+typedef struct {
+  double a, M;           /* Kerr spin and mass (M = 1 in production; M = 0: flat space) PAPER.md:433 */
+  int32_t nr, nth;       /* physical cells in ln r and theta                                        */
+  int32_t ng;            /* guard nodes on each side in r and theta (>= 2)                          */
+  double xi_in, xi_out;  /* ln r of the inner / outer physical boundary               */
+  double dphi;           /* azimuthal extent of the axisymmetric slab (Delta phi of B8/B10), 2 pi   */
+  int32_t geo_iters;     /* K: trapezoidal corrector iterations of the geodesic step  */
+  int32_t field_iters;   /* N: corrector iterations of the field step                 */
+  double beta_impl;      /* semi-implicit weight beta (alpha = 1 - beta)              */
+  int32_t damp_cells;    /* width (radial cells) of the outer damping layer; 0 = off  */
+  double damp_coef;      /* lambda_i = 1 - damp_coef * s^3, s = (i - i_start)/damp_cells in (0,1]   */
+} grpic_params;
+
+/* Particle store, structure of arrays, FP64 (contravariant x^i, covariant u_i,
+ * both at integer time steps :176).  x1 = ln r, x2 = theta, x3 = phi.  w = macro-particle
+ * weight.  cell = j*nr + i of the current position (0xFFFFFFFF once removed).
+ * flag bit0: species sign, 1 = positron (q/m = +1), 0 = electron (q/m = -1);
+ * flag bit1: removed (left through the inner or outer radial boundary). */
+typedef struct {
+  double *x1, *x2, *x3, *u1, *u2, *u3, *w;
+  uint32_t *cell, *flag;
+  int64_t n;
+} grpic_particles;
+
+typedef struct { double *Dr, *Dth, *Dph, *Br, *Bth, *Bph; } grpic_fields; /* contravariant D^i, B^i */
+typedef struct { double *Fr, *Fth, *Fph; } grpic_current;                  /* fluxes or densities   */
+
+enum {
+  GRPIC_OK = 0,
+  GRPIC_ERR_ARG = -1,       /* null pointer / out-of-range parameter                 */
+  GRPIC_ERR_CUDA = -2,      /* CUDA runtime error (no device, launch failure, ...)   */
+  GRPIC_ERR_WORKSPACE = -3, /* workspace missing or too small for this call          */
+  GRPIC_ERR_ALLOC = -4      /* could not allocate the context's own tables           */
+};
+#define GRPIC_STATUS_FAR_MOVE 1u   /* a particle moved more than one cell in a step (still deposited exactly) */
+#define GRPIC_STATUS_NONFINITE 2u  /* a particle state became NaN/Inf (particle is flagged removed)           */
+#define GRPIC_STATUS_OFFGRID 4u    /* a deposit window left the guard region (contribution dropped)           */
+
+/* Create a context: validates params, computes on the device the area elements of Eq.(8)
+ * (10-point Gauss-Legendre in xi and theta; D- and B-staggered sets) and
+ * the 1-D coordinate tables.  Blocking (synchronises once).  *out is host memory. */
+int grpic_create(const grpic_params* params, grpic_ctx** out);
+int grpic_destroy(grpic_ctx* ctx);
+
+/* Pitched layout shared by every grid array (host out-pointers). */
+int grpic_grid_layout(const grpic_ctx* ctx, int32_t* pitch, int32_t* rows, int32_t* i0, int32_t* j0);
+
+/* Copy the six area-element tables A^D_r, A^D_th, A^D_ph, A^B_r, A^B_th, A^B_ph (Eq.8; the
+ * phi areas WITHOUT dphi, i.e. dV = dphi*A^D_ph) into six caller device arrays of the grid
+ * layout.  For tests and diagnostics. */
+int grpic_get_areas(const grpic_ctx* ctx, double* const out[6], void* stream);
+
+/* Scratch memory: the caller allocates grpic_workspace_bytes(ctx, max particles) bytes of
+ * device memory and registers it; push_deposit needs none, field_step / sort / compact do. */
+size_t grpic_workspace_bytes(const grpic_ctx* ctx, int64_t n_particles);
+int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes);
+
+/* One particle step n -> n+1 for all particles not yet removed (Fig.2 :239):
+ *   gather D^n,B^n at x^n (first order, :228) -> full-dt generalised Boris (Eq.16-19, :176-200)
+ *   -> geodesic predictor + K trapezoidal correctors (Eq.12,14,15, :142-174) -> axis
+ *   reflection (:136) -> removal flag (:138) and new cell -> charge-conserving deposit of the
+ *   move x^n -> x^{n+1} (Eq.21-23, :208-233, CIC shape).
+ * Particles are updated IN PLACE.  The FLUXES  F_r = J^r A^D_r, F_th = J^th A^D_th,
+ * F_ph = J^ph dV  of the step are ACCUMULATED (+=) into `flux` (zero it first; guards and
+ * theta ghost rows receive the parts deposited beyond the domain).  `fields` must have
+ * valid guard / ghost values (grpic_field_step and grpic_fill_guards maintain them).
+ * `status` may be NULL. */
+int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
+                       grpic_current* flux, double dt, uint32_t* status, void* stream);
+
+/* Fluxes -> current densities, in place: fold the theta ghost rows onto their mirror rows
+ * (particles never cross the axis, :136), `filter_passes` passes of the (1,2,1)x(1,2,1)/16
+ * binomial filter on the fluxes (BASELINE.json config 5), then J^r = F_r/A^D_r,
+ * J^th = F_th/A^D_th, J^ph = F_ph/dV (:228).  Needs workspace when filter_passes > 0. */
+int grpic_finalize_current(grpic_ctx* ctx, grpic_current* flux_to_J, int32_t filter_passes, void* stream);
+
+/* One field step D^n,B^n -> D^{n+1},B^{n+1} in place: predictor Eq.(9), N correctors
+ * Eq.(10) (:113-128), each sweep = auxiliary fields (B9),(B11) + circulations (B8),(B10)
+ * (:478-518), axis conditions incl. Eq.(11) (:132-136), radial guards (:138), outer damping
+ * layer towards `background` (NULL = towards zero).  J may be NULL (vacuum). */
+int grpic_field_step(grpic_ctx* ctx, grpic_fields* fields, const grpic_current* J,
+                     const grpic_fields* background, double dt, void* stream);
+
+/* Impose axis values, radial guards and theta ghost rows on caller-initialised fields. */
+int grpic_fill_guards(grpic_ctx* ctx, grpic_fields* fields, void* stream);
+
+/* Circulations C_H (3) and C_E (3) of the given fields (B8)-(B11), for diagnostics/tests. */
+int grpic_circulation(grpic_ctx* ctx, const grpic_fields* fields, double* const out[6], void* stream);
+
+/* Stable sort by key = removed ? ncells : cell.  `out` receives the reordered SoA (must not
+ * alias `in`), `perm[k]` = source index of output k (may be NULL).  out->n = in->n. */
+int grpic_sort(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, uint32_t* perm, void* stream);
+
+/* Order-preserving removal of flagged particles: survivors are copied to `out` (must not
+ * alias `in`) in order; their count is written to the DEVICE word n_alive. */
+int grpic_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, int64_t* n_alive, void* stream);
+
+/* Charge density on vertices, rho_ij = sum q w S_ij(x) / dV_ij (theta ghosts folded);
+ * divide = 0 returns rho*dV.  Overwrites `rho`. */
+int grpic_deposit_rho(grpic_ctx* ctx, const grpic_particles* ptc, double* rho, int32_t divide, void* stream);
+
+/* Roofline denominator: measured FP64 pipe throughput of this device.  Runs a register-only
+ * kernel of independent DFMA chains on every SM (blocking, ~10 ms) and writes the achieved
+ * FP64 instructions (lane-operations) per second to the HOST double *dfma_per_second. */
+int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second);
+
+/* Number of CUDA kernels this library has launched in this process so far (all contexts);
+ * used by bench.py to report `gpu_launches`. */
+int64_t grpic_kernel_launches(void);
+
+const char* grpic_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GRPIC_H_ */

@@ -1,0 +1,344 @@
+// GR Maxwell field update (Eq.9-11, B8-B11) for sm_100a.
+//
+// Sweep kernel design: one warp owns 32 consecutive columns (r
+// index, the fastest dimension) and MARCHES over a chunk of theta rows.  Per row each lane
+//   1. loads the six field values of its own node (coalesced 256-byte row segments),
+//   2. computes the 14 metric coefficients of (B9)/(B11) inline from 1-D tables
+//      (one rsqrt per staggered location; no coefficient arrays in HBM),
+//   3. forms the "coefficient x field" products at the field's own location
+//      and exchanges them with its r-neighbours by warp shuffles (B9/B11 average in r only),
+//   4. forms the six auxiliary fields, exchanges H_phi,H_theta / E_phi,E_theta with r-neighbours,
+//   5. keeps the previous one/two rows of auxiliary fields in registers, so the circulations
+//      (B8)/(B10) of row j are complete when row j+1 has been formed,
+//   6. applies the predictor (9) or corrector (10) update, axis conditions (Eq.11), radial
+//      guard copies and (last sweep) the damping layer in the epilogue.
+// No shared memory, no block barrier; lanes 2..29 of each warp produce output (halo 2+2).
+#include <math.h>
+
+#include "grpic_internal.cuh"
+
+namespace {
+
+constexpr int kOutCols = 28;   // output columns per warp
+constexpr int kRowChunk = 32;  // output rows per warp
+constexpr int kWarpsPerBlock = 4;
+
+struct SweepArgs {
+  const double* in[6];    // iterate being evaluated (D^r,D^th,D^ph,B^r,B^th,B^ph)
+  const double* base[6];  // MODE 0: F^n; MODE 1: F^n + dt (alpha_i C^n - J)
+  const double* J[3];     // MODE 0 only (may be null)
+  const double* bg[6];    // damping background (last sweep; may be null)
+  double* out[6];
+  double* base_out[6];    // MODE 0: where to store the corrector base (may be null)
+  double dt, a_impl, b_impl;
+  int last;               // apply damping
+  int damp_cells;
+  double damp_coef;
+};
+
+struct Coef {  // at one staggered location
+  double q;      // alpha*gamma_rr = sqrt(1+z)
+  double al;     // alpha
+  double rho2;
+  double s;
+};
+__device__ __forceinline__ Coef coef_at(const GridDev& g, double r, double s, double c) {
+  Coef k;
+  k.rho2 = fma(g.a2 * c, c, r * r);
+  const double B = fma(2.0 * g.M, r, k.rho2);
+  const double rs = rsqrt(k.rho2 * B);
+  k.al = k.rho2 * rs;
+  k.q = B * rs;
+  k.s = s;
+  return k;
+}
+// alpha*gamma_rphi, sqrt(gamma)*beta^r, alpha*gamma_thth, alpha*gamma_phph
+__device__ __forceinline__ double c_rphi(const GridDev& g, const Coef& k) { return -g.a * k.s * k.s * k.q; }
+__device__ __forceinline__ double c_sgb(const GridDev& g, const Coef& k, double r) { return 2.0 * g.M * r * k.s * k.al; }
+__device__ __forceinline__ double c_thth(const Coef& k) { return k.rho2 * k.al; }
+__device__ __forceinline__ double c_phph(const GridDev& g, const Coef& k) {
+  const double s2 = k.s * k.s;
+  return s2 * fma(g.a2 * s2, k.q, k.rho2 * k.al);
+}
+
+__device__ __forceinline__ double shfl_up1(double v) { return __shfl_up_sync(0xffffffffu, v, 1); }
+__device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0xffffffffu, v, 1); }
+
+// MODE 0: predictor (Eq.9) + store corrector base; MODE 1: corrector (Eq.10); MODE 2: write
+// the circulations themselves (diagnostics).
+template <int MODE>
+__global__ void __launch_bounds__(32 * kWarpsPerBlock)
+field_sweep_kernel(GridDev g, SweepArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int wcol = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int ibase = wcol * kOutCols;
+  if (ibase > g.nr) return;
+  const int i = ibase - 2 + lane;                       // this lane's column
+  const int ic = min(max(i, -g.ng), g.nr + g.ng);       // clamped for loads
+  const int jstart = blockIdx.y * kRowChunk;
+  const int jend = min(jstart + kRowChunk, g.nth + 1);  // output rows [jstart, jend)
+  const bool writer = (lane >= 2) && (lane < 2 + kOutCols) && (i <= g.nr);
+
+  const double r_n = __ldg(g.r_n + ic + g.i0), r_h = __ldg(g.r_h + ic + g.i0);
+  const double dr_n = __ldg(g.dr_n + ic + g.i0), dr_h = __ldg(g.dr_h + ic + g.i0);
+
+  // previous rows of auxiliary fields
+  double Hph_p = 0, Hph_im1_p = 0, Hr_p = 0, Hth_p = 0, Hth_im1_p = 0;
+  double Eph_p = 0, Eph_ip1_p = 0, Er_p = 0, Eth_p = 0, Eth_ip1_p = 0;
+  double Hph_pp = 0, Hr_pp = 0;
+
+  for (int jj = jstart - 1; jj <= jend; ++jj) {
+    // ---- auxiliary fields of row jj ----
+    double Hph = 0, Hr = 0, Hth = 0, Eph = 0, Er = 0, Eth = 0;
+    {
+      const size_t k = g.idx(ic, jj);
+      const double Dr = __ldg(A.in[0] + k), Dth = __ldg(A.in[1] + k), Dph = __ldg(A.in[2] + k);
+      const double Br = __ldg(A.in[3] + k), Bth = __ldg(A.in[4] + k), Bph = __ldg(A.in[5] + k);
+      const double sn = __ldg(g.sin_n + jj + g.j0), cn = __ldg(g.cos_n + jj + g.j0);
+      const double sh = __ldg(g.sin_h + jj + g.j0), ch = __ldg(g.cos_h + jj + g.j0);
+      const Coef knn = coef_at(g, r_n, sn, cn), khn = coef_at(g, r_h, sn, cn);
+      const Coef knh = coef_at(g, r_n, sh, ch), khh = coef_at(g, r_h, sh, ch);
+      const double P1 = c_rphi(g, khh) * Bph, P6 = c_sgb(g, khh, r_h) * Bph;
+      const double P2 = c_sgb(g, knn, r_n) * Dph, P5 = c_rphi(g, knn) * Dph;
+      const double P3 = c_rphi(g, knh) * Br, P4 = c_sgb(g, knh, r_n) * Dth;
+      const double P7 = c_rphi(g, khn) * Dr, P8 = c_sgb(g, khn, r_h) * Bth;
+      const double P1m = shfl_up1(P1), P6m = shfl_up1(P6), P7m = shfl_up1(P7), P8m = shfl_up1(P8);
+      const double P2p = shfl_dn1(P2), P5p = shfl_dn1(P5), P3p = shfl_dn1(P3), P4p = shfl_dn1(P4);
+      const bool row_n = (jj >= 0) && (jj <= g.nth);      // node-in-theta rows
+      const bool row_h = (jj >= 0) && (jj <= g.nth - 1);  // half-in-theta rows
+      if (row_n) {
+        Hth = fma(c_thth(khn), Bth, 0.5 * (P2 + P2p));                       // (B9)
+        Er = fma(khn.q, Dr, 0.5 * (P5 + P5p));                               // (B11)
+        Eph = fma(c_phph(g, knn), Dph, 0.5 * (P7 + P7m) + 0.5 * (P8 + P8m)); // (B11), 1/2 restored
+      }
+      if (row_h) {
+        Hr = fma(knh.q, Br, 0.5 * (P1 + P1m));                               // (B9)
+        Hph = fma(c_phph(g, khh), Bph, 0.5 * (P3 + P3p) - 0.5 * (P4 + P4p)); // (B9)
+        Eth = fma(c_thth(knh), Dth, -0.5 * (P6 + P6m));                      // (B11)
+      }
+    }
+    const double Hph_im1 = shfl_up1(Hph), Hth_im1 = shfl_up1(Hth);
+    const double Eph_ip1 = shfl_dn1(Eph), Eth_ip1 = shfl_dn1(Eth);
+
+    // ---- outputs of row j = jj-1 ----
+    const int j = jj - 1;
+    if (j >= jstart && writer) {
+      const size_t k = g.idx(i, j);
+      const bool axis = (j == 0) || (j == g.nth);
+      const bool halfrow = (j < g.nth);
+      const bool halfcol = (i < g.nr);
+      double C[6];
+      C[0] = (Hph_p - Hph_pp) * __ldg(g.iADr + k);                                    // (B8), Eq.(11) on the axes
+      C[1] = (Hph_im1_p - Hph_p) * __ldg(g.iADth + k);
+      C[2] = fma(Hth_p - Hth_im1_p, g.dth, (Hr_pp - Hr_p) * dr_n) * __ldg(g.iADph + k);
+      C[3] = -(Eph - Eph_p) * __ldg(g.iABr + k);                                      // (B10)
+      C[4] = -(Eph_p - Eph_ip1_p) * __ldg(g.iABth + k);
+      C[5] = -fma(Eth_ip1_p - Eth_p, g.dth, (Er_p - Er) * dr_h) * __ldg(g.iABph + k);
+      // physical range of each component
+      const bool ok[6] = {halfcol, halfrow, !axis, halfrow, halfcol && !axis, halfcol && halfrow};
+      // i of the last physical column of each component (for the radial guard copies)
+      const int hi[6] = {g.nr - 1, g.nr, g.nr, g.nr, g.nr - 1, g.nr - 1};
+      double lam = 1.0;
+      if (A.last && A.damp_cells > 0) {
+        const int i0d = g.nr - A.damp_cells;
+        if (i > i0d) {
+          const double sd = (double)(i - i0d) / (double)(g.nr - i0d);
+          lam = 1.0 - A.damp_coef * sd * sd * sd;
+        }
+      }
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        double v;
+        const bool rowok = (c == 1 || c == 3 || c == 5) ? halfrow : true;
+        if (MODE == 2) {
+          v = ok[c] ? C[c] : 0.0;
+        } else if (MODE == 0) {
+          const double Fn = __ldg(A.base[c] + k);
+          const double Jc = (c < 3 && A.J[c]) ? __ldg(A.J[c] + k) : 0.0;
+          v = ok[c] ? fma(A.dt, C[c] - Jc, Fn) : 0.0;
+          if (A.base_out[c] && rowok && i <= hi[c])
+            A.base_out[c][k] = ok[c] ? fma(A.dt, A.a_impl * C[c] - Jc, Fn) : 0.0;
+        } else {
+          v = ok[c] ? fma(A.dt * A.b_impl, C[c], __ldg(A.base[c] + k)) : 0.0;
+        }
+        if (MODE != 2 && lam != 1.0 && ok[c]) {
+          const double b = A.bg[c] ? __ldg(A.bg[c] + k) : 0.0;
+          v = fma(v - b, lam, b);
+        }
+        if (rowok && i <= hi[c]) {
+          A.out[c][k] = v;
+          if (MODE != 2) {
+            if (i == 0)
+              for (int gq = 1; gq <= g.ng; ++gq) A.out[c][k - gq] = v;
+            if (i == hi[c])
+              for (int gq = 1; gq <= g.nr + g.ng - hi[c]; ++gq) A.out[c][k + gq] = v;
+          }
+        }
+      }
+    }
+    // ---- rotate rows ----
+    Hph_pp = Hph_p; Hr_pp = Hr_p;
+    Hph_p = Hph; Hph_im1_p = Hph_im1; Hr_p = Hr; Hth_p = Hth; Hth_im1_p = Hth_im1;
+    Eph_p = Eph; Eph_ip1_p = Eph_ip1; Er_p = Er; Eth_p = Eth; Eth_ip1_p = Eth_ip1;
+  }
+}
+
+// Axis values, radial guard copies and theta ghost rows by parity (S8); three tiny kernels.
+__device__ __forceinline__ double* comp(const grpic_fields& f, int c) {
+  return c == 0 ? f.Dr : c == 1 ? f.Dth : c == 2 ? f.Dph : c == 3 ? f.Br : c == 4 ? f.Bth : f.Bph;
+}
+// D^ph = B^th = 0 on the axis nodes: one thread per physical column.
+__global__ void axis_zero_kernel(GridDev g, grpic_fields f) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i > g.nr) return;
+  f.Dph[g.idx(i, 0)] = 0.0;
+  f.Dph[g.idx(i, g.nth)] = 0.0;
+  if (i < g.nr) {
+    f.Bth[g.idx(i, 0)] = 0.0;
+    f.Bth[g.idx(i, g.nth)] = 0.0;
+  }
+}
+// radial guards = last physical value: one thread per (row, component).
+__global__ void radial_guards_kernel(GridDev g, grpic_fields f) {
+  const int c = blockIdx.y;
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  const int hi = (c == 0 || c == 4 || c == 5) ? g.nr - 1 : g.nr;
+  const int jhi = (c == 1 || c == 3 || c == 5) ? g.nth - 1 : g.nth;
+  if (j > jhi) return;
+  double* X = comp(f, c);
+  const double lo = X[g.idx(0, j)], up = X[g.idx(hi, j)];
+  for (int i = -g.ng; i < 0; ++i) X[g.idx(i, j)] = lo;
+  for (int i = hi + 1; i <= g.nr + g.ng; ++i) X[g.idx(i, j)] = up;
+}
+// theta ghost rows by parity (r, phi components even; theta components odd): one thread per
+// (padded column, component).
+__global__ void ghost_rows_kernel(GridDev g, grpic_fields f) {
+  const int c = blockIdx.y;
+  const int i = blockIdx.x * blockDim.x + threadIdx.x - g.ng;
+  if (i > g.nr + g.ng) return;
+  const bool half_t = (c == 1 || c == 3 || c == 5);
+  const double par = (c == 1 || c == 4) ? -1.0 : 1.0;
+  double* X = comp(f, c);
+  for (int gq = 1; gq <= g.ng; ++gq) {
+    if (!half_t) {
+      X[g.idx(i, -gq)] = par * X[g.idx(i, gq)];
+      X[g.idx(i, g.nth + gq)] = par * X[g.idx(i, g.nth - gq)];
+    } else {
+      X[g.idx(i, -gq)] = par * X[g.idx(i, gq - 1)];
+      X[g.idx(i, g.nth - 1 + gq)] = par * X[g.idx(i, g.nth - gq)];
+    }
+  }
+  if (half_t) X[g.idx(i, g.nth + g.ng)] = 0.0;
+}
+
+int fill_guards(const GridDev& g, grpic_fields* f, cudaStream_t st) {
+  axis_zero_kernel<<<(g.nr + 1 + 127) / 128, 128, 0, st>>>(g, *f);
+  dim3 ga((g.nth + 1 + 127) / 128, 6);
+  radial_guards_kernel<<<ga, 128, 0, st>>>(g, *f);
+  dim3 gb((g.nr + 1 + 2 * g.ng + 127) / 128, 6);
+  ghost_rows_kernel<<<gb, 128, 0, st>>>(g, *f);
+  grpic_count_launches(3);
+  return grpic_launch_ok();
+}
+
+template <int MODE>
+int launch_sweep(const grpic_ctx* ctx, const SweepArgs& A, cudaStream_t st) {
+  const GridDev& g = ctx->g;
+  const int wcols = (g.nr + 1 + kOutCols - 1) / kOutCols;
+  dim3 grid((wcols + kWarpsPerBlock - 1) / kWarpsPerBlock, (g.nth + 1 + kRowChunk - 1) / kRowChunk);
+  field_sweep_kernel<MODE><<<grid, 32 * kWarpsPerBlock, 0, st>>>(g, A);
+  grpic_count_launches(1);
+  return grpic_launch_ok();
+}
+
+bool fields_ok(const grpic_fields* f) {
+  return f && f->Dr && f->Dth && f->Dph && f->Br && f->Bth && f->Bph;
+}
+void to_array(const grpic_fields* f, const double* out[6]) {
+  out[0] = f->Dr; out[1] = f->Dth; out[2] = f->Dph; out[3] = f->Br; out[4] = f->Bth; out[5] = f->Bph;
+}
+
+}  // namespace
+
+extern "C" {
+
+int grpic_fill_guards(grpic_ctx* ctx, grpic_fields* fields, void* stream) {
+  if (!ctx || !fields_ok(fields)) return GRPIC_ERR_ARG;
+  return fill_guards(ctx->g, fields, (cudaStream_t)stream);
+}
+
+int grpic_circulation(grpic_ctx* ctx, const grpic_fields* fields, double* const out[6], void* stream) {
+  if (!ctx || !fields_ok(fields) || !out) return GRPIC_ERR_ARG;
+  SweepArgs A = {};
+  to_array(fields, A.in);
+  for (int c = 0; c < 6; ++c) {
+    if (!out[c]) return GRPIC_ERR_ARG;
+    A.out[c] = out[c];
+  }
+  return launch_sweep<2>(ctx, A, (cudaStream_t)stream);
+}
+
+int grpic_field_step(grpic_ctx* ctx, grpic_fields* fields, const grpic_current* J,
+                     const grpic_fields* background, double dt, void* stream) {
+  if (!ctx || !fields_ok(fields) || !(dt >= 0.0)) return GRPIC_ERR_ARG;
+  if (background && !fields_ok(background)) return GRPIC_ERR_ARG;
+  if (J && (!J->Fr || !J->Fth || !J->Fph)) return GRPIC_ERR_ARG;
+  const GridDev& g = ctx->g;
+  const size_t n2 = g.size();
+  if (!ctx->ws || ctx->ws_bytes < 18 * n2 * sizeof(double)) return GRPIC_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)stream;
+  double* ws = (double*)ctx->ws;
+  double* base[6];
+  double* itA[6];
+  double* itB[6];
+  for (int c = 0; c < 6; ++c) {
+    base[c] = ws + (size_t)c * n2;
+    itA[c] = ws + (size_t)(6 + c) * n2;
+    itB[c] = ws + (size_t)(12 + c) * n2;
+  }
+  double* F[6] = {fields->Dr, fields->Dth, fields->Dph, fields->Br, fields->Bth, fields->Bph};
+  int rc = fill_guards(g, fields, st);
+  if (rc != GRPIC_OK) return rc;
+  const int N = ctx->p.field_iters;
+  SweepArgs A = {};
+  A.dt = dt;
+  A.b_impl = ctx->p.beta_impl;
+  A.a_impl = 1.0 - ctx->p.beta_impl;
+  A.damp_cells = ctx->p.damp_cells;
+  A.damp_coef = ctx->p.damp_coef;
+  if (background) to_array(background, A.bg);
+  // predictor, Eq.(9)
+  for (int c = 0; c < 6; ++c) {
+    A.in[c] = F[c];
+    A.base[c] = F[c];
+    A.out[c] = itA[c];
+    A.base_out[c] = (N > 0) ? base[c] : nullptr;
+  }
+  if (J) { A.J[0] = J->Fr; A.J[1] = J->Fth; A.J[2] = J->Fph; }
+  A.last = (N == 0);
+  rc = launch_sweep<0>(ctx, A, st);
+  if (rc != GRPIC_OK) return rc;
+  if (N == 0) {
+    for (int c = 0; c < 6; ++c)
+      GRPIC_CUDA_OK(cudaMemcpyAsync(F[c], itA[c], n2 * sizeof(double), cudaMemcpyDeviceToDevice, st));
+  }
+  // correctors, Eq.(10); the last one writes the caller's arrays
+  double** cur = itA;
+  double** nxt = itB;
+  for (int it = 0; it < N; ++it) {
+    const bool last = (it == N - 1);
+    for (int c = 0; c < 6; ++c) {
+      A.in[c] = cur[c];
+      A.base[c] = base[c];
+      A.out[c] = last ? F[c] : nxt[c];
+      A.base_out[c] = nullptr;
+    }
+    A.last = last;
+    rc = launch_sweep<1>(ctx, A, st);
+    if (rc != GRPIC_OK) return rc;
+    double** t = cur; cur = nxt; nxt = t;
+  }
+  return fill_guards(g, fields, st);
+}
+
+}  // extern "C"

@@ -1,0 +1,337 @@
+// Particle cell-sort (stable LSD radix sort on the cell key) and order-preserving compaction
+// of removed particles, with warp-level match/ballot ranking.  Hand-written for sm_100a; no
+// CUB/Thrust.  Sort is not part of the paper (BASELINE.json north_star); removal follows
+// PAPER.md:138,:364.
+#include "grpic_internal.cuh"
+
+namespace {
+
+constexpr int kTile = 2048;     // keys per block
+constexpr int kThreads = 256;   // 8 warps, each owns 256 consecutive keys = 8 groups of 32
+constexpr int kGroups = 8;
+constexpr int kRadix = 256;
+
+// ------------------------------------------------------------------ device-wide exclusive scan
+constexpr int kScanTile = 2048;
+__device__ __forceinline__ uint32_t warp_incl_scan(uint32_t v, int lane) {
+#pragma unroll
+  for (int d = 1; d < 32; d <<= 1) {
+    const uint32_t t = __shfl_up_sync(0xffffffffu, v, d);
+    if (lane >= d) v += t;
+  }
+  return v;
+}
+// exclusive scan of one 2048-element tile held 8 per thread (blocked); returns tile total
+__device__ __forceinline__ uint32_t block_excl_scan8(uint32_t v[8], uint32_t* smem /*>=9*/) {
+  uint32_t sum = 0;
+#pragma unroll
+  for (int m = 0; m < 8; ++m) sum += v[m];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const uint32_t incl = warp_incl_scan(sum, lane);
+  if (lane == 31) smem[w] = incl;
+  __syncthreads();
+  if (w == 0) {
+    const uint32_t ws = (lane < 8) ? smem[lane] : 0u;
+    const uint32_t wi = warp_incl_scan(ws, lane);
+    if (lane < 8) smem[lane] = wi - ws;
+    if (lane == 7) smem[8] = wi;
+  }
+  __syncthreads();
+  uint32_t run = smem[w] + incl - sum;
+#pragma unroll
+  for (int m = 0; m < 8; ++m) {
+    const uint32_t t = v[m];
+    v[m] = run;
+    run += t;
+  }
+  return smem[8];
+}
+__global__ void __launch_bounds__(kThreads) scan_tiles_kernel(uint32_t* data, size_t n, uint32_t* sums) {
+  __shared__ uint32_t sm[9];
+  const size_t base = (size_t)blockIdx.x * kScanTile + (size_t)threadIdx.x * 8;
+  uint32_t v[8];
+#pragma unroll
+  for (int m = 0; m < 8; ++m) v[m] = (base + m < n) ? data[base + m] : 0u;
+  const uint32_t tot = block_excl_scan8(v, sm);
+#pragma unroll
+  for (int m = 0; m < 8; ++m)
+    if (base + m < n) data[base + m] = v[m];
+  if (threadIdx.x == 0 && sums) sums[blockIdx.x] = tot;
+}
+__global__ void __launch_bounds__(kThreads) scan_add_kernel(uint32_t* data, size_t n, const uint32_t* sums) {
+  const uint32_t off = sums[blockIdx.x];
+  const size_t base = (size_t)blockIdx.x * kScanTile + (size_t)threadIdx.x * 8;
+#pragma unroll
+  for (int m = 0; m < 8; ++m)
+    if (base + m < n) data[base + m] += off;
+}
+// In-place exclusive scan of data[0..n); scratch must hold >= n/2048 + n/2048^2 + 8 words.
+int exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st) {
+  const size_t nb = (n + kScanTile - 1) / kScanTile;
+  if (nb <= 1) {
+    scan_tiles_kernel<<<1, kThreads, 0, st>>>(data, n, nullptr);
+    grpic_count_launches(1);
+    return grpic_launch_ok();
+  }
+  grpic_count_launches(2);
+  scan_tiles_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
+  int rc = exclusive_scan(scratch, nb, scratch + nb, st);
+  if (rc != GRPIC_OK) return rc;
+  scan_add_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
+  return grpic_launch_ok();
+}
+
+// ------------------------------------------------------------------ radix sort passes
+__device__ __forceinline__ uint32_t make_key(uint32_t cell, uint32_t flag, uint32_t ncells) {
+  return (flag & 2u) ? ncells : min(cell, ncells);
+}
+
+// per-tile digit histogram -> hist[digit*ntiles + tile]
+template <bool FIRST>
+__global__ void __launch_bounds__(kThreads)
+radix_hist_kernel(const uint32_t* keys, const uint32_t* cell, const uint32_t* flag, int64_t n,
+                  uint32_t ncells, int shift, uint32_t* hist, uint32_t ntiles) {
+  __shared__ uint32_t sh[kRadix];
+  sh[threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t base = (int64_t)blockIdx.x * kTile;
+#pragma unroll
+  for (int m = 0; m < kTile / kThreads; ++m) {
+    const int64_t e = base + m * kThreads + threadIdx.x;
+    if (e < n) {
+      const uint32_t key = FIRST ? make_key(cell[e], flag[e], ncells) : keys[e];
+      atomicAdd(&sh[(key >> shift) & 0xFFu], 1u);
+    }
+  }
+  __syncthreads();
+  hist[(size_t)threadIdx.x * ntiles + blockIdx.x] = sh[threadIdx.x];
+}
+
+// stable scatter of one tile: warp w owns keys [w*256, w*256+256) of the tile in 8 groups
+template <bool FIRST>
+__global__ void __launch_bounds__(kThreads)
+radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint32_t* cell,
+                     const uint32_t* flag, int64_t n, uint32_t ncells, int shift,
+                     const uint32_t* hist_scanned, uint32_t ntiles, uint32_t* keys_out,
+                     uint32_t* idx_out) {
+  __shared__ uint32_t whist[kThreads / 32][kRadix];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+  for (int q = 0; q < kThreads / 32; ++q) whist[q][threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t wbase = (int64_t)blockIdx.x * kTile + (int64_t)w * (kGroups * 32);
+  uint32_t key[kGroups], idx[kGroups], dig[kGroups];
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const int64_t e = wbase + q * 32 + lane;
+    if (e < n) {
+      key[q] = FIRST ? make_key(cell[e], flag[e], ncells) : keys_in[e];
+      idx[q] = FIRST ? (uint32_t)e : idx_in[e];
+      dig[q] = (key[q] >> shift) & 0xFFu;
+    } else {
+      key[q] = 0; idx[q] = 0; dig[q] = 0x100u;   // sentinel: never ranked or written
+    }
+  }
+  // 1. per-warp digit counts
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const uint32_t peers = __match_any_sync(0xffffffffu, dig[q]);
+    if (dig[q] < kRadix && lane == (__ffs(peers) - 1)) whist[w][dig[q]] += __popc(peers);
+    __syncwarp();
+  }
+  __syncthreads();
+  // 2. digit t: global start of each warp's run = scanned histogram + counts of earlier warps
+  {
+    uint32_t run = hist_scanned[(size_t)threadIdx.x * ntiles + blockIdx.x];
+#pragma unroll
+    for (int q = 0; q < kThreads / 32; ++q) {
+      const uint32_t cnt = whist[q][threadIdx.x];
+      whist[q][threadIdx.x] = run;
+      run += cnt;
+    }
+  }
+  __syncthreads();
+  // 3. rank inside the warp, group by group (keeps the input order of equal digits)
+  const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const uint32_t peers = __match_any_sync(0xffffffffu, dig[q]);
+    uint32_t pos = 0;
+    if (dig[q] < kRadix) pos = whist[w][dig[q]] + __popc(peers & lt);
+    __syncwarp();
+    if (dig[q] < kRadix && lane == (__ffs(peers) - 1)) whist[w][dig[q]] += __popc(peers);
+    __syncwarp();
+    if (dig[q] < kRadix) {
+      keys_out[pos] = key[q];
+      idx_out[pos] = idx[q];
+    }
+  }
+}
+
+__global__ void gather_particles_kernel(grpic_particles in, grpic_particles out, const uint32_t* perm,
+                                        uint32_t* perm_out) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= in.n) return;
+  const uint32_t s = perm[k];
+  out.x1[k] = in.x1[s]; out.x2[k] = in.x2[s]; out.x3[k] = in.x3[s];
+  out.u1[k] = in.u1[s]; out.u2[k] = in.u2[s]; out.u3[k] = in.u3[s];
+  out.w[k] = in.w[s];
+  out.cell[k] = in.cell[s];
+  out.flag[k] = in.flag[s];
+  if (perm_out) perm_out[k] = s;
+}
+
+// ------------------------------------------------------------------ compaction
+__global__ void __launch_bounds__(kThreads)
+alive_count_kernel(const uint32_t* flag, int64_t n, uint32_t* counts) {
+  __shared__ uint32_t sm[kThreads / 32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int64_t wbase = (int64_t)blockIdx.x * kTile + (int64_t)w * (kGroups * 32);
+  uint32_t c = 0;
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const int64_t e = wbase + q * 32 + lane;
+    const bool alive = (e < n) && !(flag[e] & 2u);
+    c += __popc(__ballot_sync(0xffffffffu, alive));
+  }
+  if (lane == 0) sm[w] = c;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t t = 0;
+    for (int q = 0; q < kThreads / 32; ++q) t += sm[q];
+    counts[blockIdx.x] = t;
+  }
+}
+
+__global__ void __launch_bounds__(kThreads)
+compact_scatter_kernel(grpic_particles in, grpic_particles out, const uint32_t* offsets,
+                       uint32_t ntiles, int64_t* n_alive) {
+  __shared__ uint32_t sm[kThreads / 32];
+  const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+  const int64_t wbase = (int64_t)blockIdx.x * kTile + (int64_t)w * (kGroups * 32);
+  uint32_t ballots[kGroups];
+  uint32_t c = 0;
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const int64_t e = wbase + q * 32 + lane;
+    const bool alive = (e < in.n) && !(in.flag[e] & 2u);
+    ballots[q] = __ballot_sync(0xffffffffu, alive);
+    c += __popc(ballots[q]);
+  }
+  if (lane == 0) sm[w] = c;
+  __syncthreads();
+  uint32_t off = offsets[blockIdx.x];
+  uint32_t tile_total = 0;
+  for (int q = 0; q < kThreads / 32; ++q) {
+    if (q < w) off += sm[q];
+    tile_total += sm[q];
+  }
+  if (blockIdx.x == ntiles - 1 && threadIdx.x == 0)
+    *n_alive = (int64_t)offsets[blockIdx.x] + (int64_t)tile_total;
+  const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const int64_t e = wbase + q * 32 + lane;
+    if (ballots[q] & (1u << lane)) {
+      const uint32_t d = off + __popc(ballots[q] & lt);
+      out.x1[d] = in.x1[e]; out.x2[d] = in.x2[e]; out.x3[d] = in.x3[e];
+      out.u1[d] = in.u1[e]; out.u2[d] = in.u2[e]; out.u3[d] = in.u3[e];
+      out.w[d] = in.w[e];
+      out.cell[d] = in.cell[e];
+      out.flag[d] = in.flag[e];
+    }
+    off += __popc(ballots[q]);
+  }
+}
+// entries [n_alive, n) of the output are marked removed, so the caller may keep using n as an
+// upper bound without reading n_alive back.
+__global__ void mark_tail_kernel(grpic_particles out, int64_t n, const int64_t* n_alive) {
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < n && k >= *n_alive) {
+    out.flag[k] = 2u;
+    out.cell[k] = 0xFFFFFFFFu;
+  }
+}
+
+bool ptc_ok(const grpic_particles* p) {
+  return p && p->n >= 0 &&
+         (p->n == 0 || (p->x1 && p->x2 && p->x3 && p->u1 && p->u2 && p->u3 && p->w && p->cell && p->flag));
+}
+
+}  // namespace
+
+extern "C" {
+
+int grpic_sort(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, uint32_t* perm, void* stream) {
+  if (!ctx || !ptc_ok(in) || !out) return GRPIC_ERR_ARG;
+  const int64_t n = in->n;
+  out->n = n;
+  if (n == 0) return GRPIC_OK;
+  if (!ptc_ok(out) || out->x1 == in->x1 || n > 0xFFFFFFF0LL) return GRPIC_ERR_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t nA = ((size_t)n + 63) & ~(size_t)63;
+  const uint32_t ntiles = (uint32_t)((n + kTile - 1) / kTile);
+  const size_t nh = (size_t)kRadix * ntiles;
+  const size_t need = (4 * nA + nh + nh / kScanTile + 4096) * sizeof(uint32_t);
+  if (!ctx->ws || ctx->ws_bytes < need) return GRPIC_ERR_WORKSPACE;
+  uint32_t* kA = (uint32_t*)ctx->ws;
+  uint32_t* kB = kA + nA;
+  uint32_t* iA = kB + nA;
+  uint32_t* iB = iA + nA;
+  uint32_t* hist = iB + nA;
+  uint32_t* scratch = hist + nh;
+  const uint32_t ncells = (uint32_t)ctx->g.nr * (uint32_t)ctx->g.nth;
+  int bits = 0;
+  while ((1ull << bits) <= (unsigned long long)ncells) ++bits;   // keys in [0, ncells]
+  const int passes = (bits + 7) / 8;
+  uint32_t *kin = kA, *kout = kB, *iin = iA, *iout = iB;
+  for (int p = 0; p < passes; ++p) {
+    const int shift = 8 * p;
+    if (p == 0) {
+      radix_hist_kernel<true><<<ntiles, kThreads, 0, st>>>(nullptr, in->cell, in->flag, n, ncells, shift, hist, ntiles);
+    } else {
+      radix_hist_kernel<false><<<ntiles, kThreads, 0, st>>>(kin, nullptr, nullptr, n, ncells, shift, hist, ntiles);
+    }
+    int rc = exclusive_scan(hist, nh, scratch, st);
+    if (rc != GRPIC_OK) return rc;
+    if (p == 0) {
+      radix_scatter_kernel<true><<<ntiles, kThreads, 0, st>>>(nullptr, nullptr, in->cell, in->flag, n, ncells,
+                                                              shift, hist, ntiles, kout, iout);
+    } else {
+      radix_scatter_kernel<false><<<ntiles, kThreads, 0, st>>>(kin, iin, nullptr, nullptr, n, ncells, shift,
+                                                               hist, ntiles, kout, iout);
+    }
+    uint32_t* t = kin; kin = kout; kout = t;
+    t = iin; iin = iout; iout = t;
+    grpic_count_launches(2);
+  }
+  grpic_count_launches(1);
+  gather_particles_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(*in, *out, iin, perm);
+  return grpic_launch_ok();
+}
+
+int grpic_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, int64_t* n_alive, void* stream) {
+  if (!ctx || !ptc_ok(in) || !out || !n_alive) return GRPIC_ERR_ARG;
+  const int64_t n = in->n;
+  out->n = n;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) {
+    GRPIC_CUDA_OK(cudaMemsetAsync(n_alive, 0, sizeof(int64_t), st));
+    return GRPIC_OK;
+  }
+  if (!ptc_ok(out) || out->x1 == in->x1 || n > 0xFFFFFFF0LL) return GRPIC_ERR_ARG;
+  const uint32_t ntiles = (uint32_t)((n + kTile - 1) / kTile);
+  const size_t need = ((size_t)ntiles + ntiles / kScanTile + 4096) * sizeof(uint32_t);
+  if (!ctx->ws || ctx->ws_bytes < need) return GRPIC_ERR_WORKSPACE;
+  uint32_t* counts = (uint32_t*)ctx->ws;
+  uint32_t* scratch = counts + ntiles;
+  alive_count_kernel<<<ntiles, kThreads, 0, st>>>(in->flag, n, counts);
+  int rc = exclusive_scan(counts, ntiles, scratch, st);
+  if (rc != GRPIC_OK) return rc;
+  compact_scatter_kernel<<<ntiles, kThreads, 0, st>>>(*in, *out, counts, ntiles, n_alive);
+  mark_tail_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(*out, n, n_alive);
+  grpic_count_launches(3);
+  return grpic_launch_ok();
+}
+
+}  // extern "C"
