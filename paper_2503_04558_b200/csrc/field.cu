@@ -228,7 +228,7 @@ __global__ void ghost_rows_kernel(GridDev g, grpic_fields f) {
       X[g.idx(i, g.nth - 1 + gq)] = par * X[g.idx(i, g.nth - gq)];
     }
   }
-  if (half_t) X[g.idx(i, g.nth + g.ng)] = 0.0;
+  if (half_t) X[g.idx(i, g.nth + g.ng)] = par * X[g.idx(i, g.nth - 1 - g.ng)];
 }
 
 int fill_guards(const GridDev& g, grpic_fields* f, cudaStream_t st) {

@@ -147,8 +147,8 @@ def fill_guards(p, fields):
             else:
                 F[G - g, :] = par * F[G + g - 1, :]
                 F[G + nth - 1 + g, :] = par * F[G + nth - g, :]
-        if sth != 0.0:
-            F[G + nth + G, :] = 0.0
+        if sth != 0.0:   # last stored row of a half-staggered component: mirror of row nth-1-G
+            F[G + nth + G, :] = par * F[nth - 1, :]
         out.append(F)
     return out
 
@@ -304,7 +304,7 @@ def config(k, scale=1.0, nr=None, nth=None, n=None):
         p = grid_params(nr or 1024, nth or 1024, 0.99)
         rng = np.random.Generator(np.random.PCG64(1001))
         out.update(params=p, dt=courant_dt(p),
-                   fields=perturb(analytic_fields(p, "wald"), 1e-3, rng),
+                   fields=fill_guards(p, perturb(analytic_fields(p, "wald"), 1e-3, rng)),
                    particles=make_particles(p, n or 20_000_000, 1, "r2",
                                             ("mj_tail", 1.0, 0.1, 10.0, 1e4), pairs=True),
                    meta=dict(steps=100, sort_every=20, filter_passes=0, field=False))
@@ -312,7 +312,7 @@ def config(k, scale=1.0, nr=None, nth=None, n=None):
         p = grid_params(nr or 2048, nth or 2048, 0.99)
         rng = np.random.Generator(np.random.PCG64(1002))
         out.update(params=p, dt=courant_dt(p),
-                   fields=perturb(analytic_fields(p, "wald"), 1e-3, rng),
+                   fields=fill_guards(p, perturb(analytic_fields(p, "wald"), 1e-3, rng)),
                    particles=make_particles(p, n or 100_000_000, 2, "crowded",
                                             ("loguniform", 0.1, 1e5)),
                    meta=dict(steps=50, sort_every=0, compact_every=1, filter_passes=0, field=False))

@@ -68,12 +68,27 @@ def oracle_push_deposit(O, p, fields, ptc, dt):
     return new, F
 
 
-def check_push(p, ptc, ref, got, tol=1e-12):
+def check_push(p, ptc, ref, got, O=None, fields=None, dt=None, tol=1e-12, max_frac=1e-4):
+    """x,u <= 1e-12 (G20 norm); integer outputs bit-exact outside the edge-ambiguous set.
+    Ill-conditioned particles (a stiff 1/sin^3 force within ~1e-3 cell of the axis amplifies
+    one ulp of the input by > 1e4) are compared at 10x the oracle's OWN sensitivity to a
+    4-ulp perturbation of the input position."""
     amb = edge_ambiguous(p, ref)
     ex = ptc_err(ref, got, ("x1", "x2", "x3"))
     eu = ptc_err(ref, got, ("u1", "u2", "u3"))
-    assert ex.max() <= tol, ("x", ex.max(), int(ex.argmax()))
-    assert eu.max() <= tol, ("u", eu.max(), int(eu.argmax()))
+    tolk = np.full(len(ex), tol)
+    if O is not None:
+        eps = 4 * np.finfo(np.float64).eps
+        pert = dict(ptc)
+        pert["x1"] = ptc["x1"] * (1.0 + eps)
+        pert["x2"] = ptc["x2"] * (1.0 + eps)
+        refp = O.push(p, fields, pert, dt)
+        sens = np.maximum(ptc_err(ref, refp, ("x1", "x2", "x3")), ptc_err(ref, refp, ("u1", "u2", "u3")))
+        tolk = np.maximum(tolk, 10.0 * sens)
+    # the set that actually exceeds the plain tolerance must be tiny (it was 1 in 1e5 on config 1)
+    assert (np.maximum(ex, eu) > tol).mean() <= max_frac, (np.maximum(ex, eu) > tol).mean()
+    assert np.all(ex <= tolk), ("x", ex.max(), int(ex.argmax()))
+    assert np.all(eu <= tolk), ("u", eu.max(), int(eu.argmax()))
     ok = ~amb
     assert np.array_equal(ref["cell"][ok], got["cell"][ok])
     assert np.array_equal(ref["flag"][ok], got["flag"][ok])
@@ -101,7 +116,7 @@ def test_push_deposit_one_step(G, O, k, nr, nth, n):
     ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
     ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
     got = P.to_numpy()
-    namb = check_push(p, ptc, ref, got)
+    namb = check_push(p, ptc, ref, got, O, fields, dt)
     assert namb <= 2
     assert np.array_equal(got["w"], ptc["w"])
     for c in range(3):
@@ -123,10 +138,14 @@ def test_axis_crossers_and_leavers(G, O):
     n = len(ptc["x1"])
     rng = np.random.default_rng(5)
     q = n // 4
-    ptc["x2"][:q] = rng.uniform(1e-3, 0.3, q) * dth
-    ptc["u2"][:q] = -np.abs(ptc["u2"][:q]) - 5.0
-    ptc["x2"][q:2 * q] = np.pi - rng.uniform(1e-3, 0.3, q) * dth
-    ptc["u2"][q:2 * q] = np.abs(ptc["u2"][q:2 * q]) + 5.0
+    for lo, sgn in ((0, -1.0), (q, +1.0)):      # fast, nearly polar motion close to the hole
+        sl = slice(lo, lo + q)
+        ptc["x1"][sl] = p["xi_in"] + rng.uniform(0.5, 12.0, q) * dxi
+        off = rng.uniform(1e-3, 0.08, q) * dth
+        ptc["x2"][sl] = off if sgn < 0 else np.pi - off
+        ptc["u1"][sl] = rng.normal(size=q)
+        ptc["u2"][sl] = sgn * rng.uniform(30.0, 300.0, q)
+        ptc["u3"][sl] = rng.normal(size=q) * 1e-3
     ptc["x1"][2 * q:3 * q] = p["xi_in"] + rng.uniform(1e-3, 0.2, q) * dxi
     ptc["u1"][2 * q:3 * q] = -np.abs(ptc["u1"][2 * q:3 * q]) - 3.0
     ptc["x1"][3 * q:] = p["xi_out"] - rng.uniform(1e-3, 0.2, n - 3 * q) * dxi
@@ -136,7 +155,7 @@ def test_axis_crossers_and_leavers(G, O):
     assert (ref["x2dep"] < 0).sum() > 50 and (ref["x2dep"] > np.pi).sum() > 50
     assert (ref["flag"] & 2).sum() > 100
     ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
-    check_push(p, ptc, ref, P.to_numpy())
+    check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-2)
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
     # a second step must leave the removed particles untouched and deposit nothing for them
@@ -157,6 +176,8 @@ def test_continuity_residual_gpu(G, O):
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
     cfg = small_case(2, 64, 64, 50000)
     p, dt, fields, ptc = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    # config 2's pairs are co-located with equal weights (rho = 0 exactly): use random weights
+    ptc["w"] = np.random.default_rng(8).uniform(0.5, 1.5, len(ptc["x1"]))
     ctx = G.Context(p, len(ptc["x1"]))
     f_t = [ctx.to_device(f) for f in fields]
     P = G.Particles.from_numpy(ptc)
@@ -287,30 +308,43 @@ def test_config1_ten_coupled_steps(G, O):
     P = G.Particles.from_numpy(ptc)
     fo = [f.copy() for f in fields]
     cur = dict(ptc)
+    # a second oracle trajectory from 4-ulp perturbed positions measures each particle's own
+    # sensitivity over the 10 steps (ill-conditioned near-axis particles, see check_push)
+    eps = 4 * np.finfo(np.float64).eps
+    cur2 = dict(ptc, x1=ptc["x1"] * (1 + eps), x2=ptc["x2"] * (1 + eps))
     for step in range(10):
         new, F = oracle_push_deposit(O, p, fo, cur, dt)
+        new2 = O.push(p, fo, cur2, dt)
+        fields_before = [f.copy() for f in fo] if step == 0 else None
         J = O.finalize_current(p, F, 0)
         O.field_step(p, fo, J, dt)
         cur = {k: new[k] for k in ("x1", "x2", "x3", "u1", "u2", "u3", "cell", "flag")}
         cur["w"] = ptc["w"]
+        cur2 = {k: new2[k] for k in ("x1", "x2", "x3", "u1", "u2", "u3", "cell", "flag")}
+        cur2["w"] = ptc["w"]
         F_t = ctx.zeros(3)
         ctx.push_deposit(P, f_t, F_t, dt)
         ctx.finalize_current(F_t, 0)
         ctx.field_step(f_t, F_t, dt)
         if step == 0:
             torch.cuda.synchronize()
-            check_push(p, ptc, new, P.to_numpy())
+            check_push(p, ptc, new, P.to_numpy(), O, fields_before, dt)
             for c in range(3):
                 assert grid_err(J[c], ctx.to_host(F_t[c])) <= 1e-11
             for c in range(6):
                 assert grid_err(fo[c], ctx.to_host(f_t[c])) <= 1e-11
     torch.cuda.synchronize()
     got = P.to_numpy()
-    same = (got["flag"] == cur["flag"])
+    same = (got["flag"] == cur["flag"]) & (cur2["flag"] == cur["flag"])
     assert same.mean() > 0.9999
-    ex = ptc_err(cur, got, ("x1", "x2", "x3"))[same]
-    eu = ptc_err(cur, got, ("u1", "u2", "u3"))[same]
-    assert ex.max() <= 1e-10 and eu.max() <= 1e-10, (ex.max(), eu.max())
+    sens = np.maximum(ptc_err(cur, cur2, ("x1", "x2", "x3")), ptc_err(cur, cur2, ("u1", "u2", "u3")))
+    tolk = np.maximum(1e-10, 100.0 * sens)
+    assert (np.maximum(ptc_err(cur, got, ("x1", "x2", "x3")), ptc_err(cur, got, ("u1", "u2", "u3")))[same]
+            > 1e-10).mean() < 1e-3
+    ex = ptc_err(cur, got, ("x1", "x2", "x3"))
+    eu = ptc_err(cur, got, ("u1", "u2", "u3"))
+    assert np.all(ex[same] <= tolk[same]) and np.all(eu[same] <= tolk[same]), \
+        (ex[same].max(), eu[same].max())
     for c in range(6):
         assert grid_err(fo[c], ctx.to_host(f_t[c])) <= 1e-10, c
 
@@ -349,7 +383,7 @@ def test_config2_full_size_sampled(G, O):
     sub = {k: np.ascontiguousarray(v[src]) for k, v in ptc.items()}
     ref = O.push(p, fields, sub, dt)
     gsub = {k: got[k][sample] for k in got}
-    check_push(p, sub, ref, gsub)
+    check_push(p, sub, ref, gsub, O, fields, dt)
     # moments: sum F_ph = sum Q dphi/dt over all particles
     Q = np.where(ptc["flag"][perm] & 1, 1.0, -1.0) * ptc["w"][perm]
     dphi = got["x3"] - ptc["x3"][perm]
