@@ -150,7 +150,7 @@ int grpic_create(const grpic_params* p, grpic_ctx** out) {
   ctx->ws_bytes = 0;
   cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
   GridDev& g = ctx->g;
-  g.a = p->a; g.M = p->M; g.a2 = p->a * p->a;
+  g.a = p->a; g.M = p->M; g.a2 = p->a * p->a; g.twoM = 2.0 * p->M;
   g.xi_in = p->xi_in; g.xi_out = p->xi_out;
   g.dxi = (p->xi_out - p->xi_in) / p->nr;
   g.dth = M_PI / p->nth;

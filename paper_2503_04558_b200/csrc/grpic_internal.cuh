@@ -7,7 +7,7 @@
 
 // Geometry + table pointers handed to every kernel by value.
 struct GridDev {
-  double a, M, a2;
+  double a, M, a2, twoM;
   double xi_in, xi_out, dxi, dth, inv_dxi, inv_dth, dphi;
   int nr, nth, ng;
   int pitch, rows, i0, j0;  // element (i,j) at (j+j0)*pitch + (i+i0)

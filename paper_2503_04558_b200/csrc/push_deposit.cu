@@ -2,41 +2,82 @@
 //
 // One thread per particle.  All Kerr-Schild metric terms (lapse, shift, spatial metric, inverse
 // metric and the r/theta derivatives entering Eq.12) are computed inline in registers from
-// (r, sin theta, cos theta); position-only terms are shared between the Boris rotation and
-// the first geodesic right-hand side.  Closed forms: Appendix A with M
-// restored; derivative forms are this file's own.
+// (r, sin theta, cos theta) with ONE reciprocal per evaluation point; position-only terms are
+// shared between the Boris rotation and the first geodesic right-hand side.  The corrector
+// iterates get sin/cos by angle addition from the start point and the new ln r by a short
+// atanh series, so a particle-step costs one exp, one sincos and no log on the common path.
+// Closed forms: Appendix A with M restored; derivative forms are this
+// file's own.
+//
+// Deposit (Eq.21-23): every particle produces the fluxes of its move on the
+// 4x4 node window anchored one node below its OLD cell (12 F_r faces, 12 F_theta faces, 16
+// F_phi nodes).  Particles are cell-sorted, so the lanes of a warp form a few runs of equal
+// window anchor.  Each warp transposes its 32 x 40 contributions through a private
+// shared-memory tile (slot-major, padded to 33), lane L then sums slot L over each run in
+// particle order and issues ONE red.global.add.f64 per (run, slot).  Warps with many runs
+// (unsorted or very sparse input) fall back to per-lane reductions of their non-zero values.
 #include <math.h>
 
 #include "grpic_internal.cuh"
 
 namespace {
 
+constexpr int kBlock = 128;
+constexpr int kSlotsA = 24;          // phase A: 12 F_r + 12 F_theta slots
+constexpr int kSlotsB = 16;          // phase B: 16 F_phi slots
+constexpr int kPad = 33;             // particles per slot row (+1 against bank conflicts)
+constexpr unsigned kFull = 0xffffffffu;
+constexpr int kDirectRuns = 12;      // more runs than this in a warp: per-lane reductions
+
+// 1/x: MUFU.RCP64H seed + two Newton steps (~1 ulp); no special-case slow path.
+__device__ __forceinline__ double rcp_nr(double x) {
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  double e = fma(-x, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-x, y, 1.0);
+  return fma(y, e, y);
+}
+// 1/sqrt(x): MUFU.RSQ64H seed + two Newton steps.
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = 0.5 * x;
+  double e = fma(-(h * y), y, 0.5);
+  y = fma(y, e, y);
+  e = fma(-(h * y), y, 0.5);
+  return fma(y, e, y);
+}
+
 struct Pos {          // position-only terms at (r, theta)
   double r, s, c;     // r, sin, cos
+  double rho2;
   double R;           // 1/rho^2
   double is2;         // 1/sin^2
-  double is;          // 1/sin
   double beta;        // beta^r = 2Mr/(rho^2+2Mr)
   double zp1;         // 1+z
   double h;           // 1/(1+z) = alpha^2
   double r2a2;        // r^2 + a^2
-  double rho2;
 };
 
 __device__ __forceinline__ Pos make_pos(const GridDev& g, double r, double s, double c) {
   Pos p;
   p.r = r; p.s = s; p.c = c;
-  p.rho2 = fma(g.a2 * c, c, r * r);
-  const double twoMr = 2.0 * g.M * r;
+  const double r2 = r * r;
+  p.rho2 = fma(g.a2 * c, c, r2);
+  const double twoMr = g.twoM * r;
   const double B = p.rho2 + twoMr;          // rho^2 (1+z)
-  p.R = 1.0 / p.rho2;
-  const double iB = 1.0 / B;
-  p.is = 1.0 / s;
-  p.is2 = p.is * p.is;
+  const double s2 = s * s;
+  const double rb = p.rho2 * B;
+  const double inv = rcp_nr(rb * s2);       // the one reciprocal: 1/(rho^2 B sin^2)
+  const double irb = inv * s2;              // 1/(rho^2 B)
+  p.R = irb * B;
+  const double iB = irb * p.rho2;
+  p.is2 = inv * rb;
   p.beta = twoMr * iB;
   p.h = p.rho2 * iB;
   p.zp1 = B * p.R;
-  p.r2a2 = fma(r, r, g.a2);
+  p.r2a2 = r2 + g.a2;
   return p;
 }
 
@@ -46,25 +87,28 @@ __device__ __forceinline__ void geodesic_rhs(const GridDev& g, const Pos& p, dou
                                              double& Ur, double& Ut) {
   const double R = p.R, R2 = R * R;
   const double ur2 = ur * ur, up2s = up * up * p.is2;
+  const double aup = g.a * up;
   // P = rho^2 * (gamma^ij u_i u_j + beta u_r^2)
-  const double P = fma(p.r2a2, ur2, fma(ut, ut, fma(2.0 * g.a * ur, up, up2s)));
+  const double P = fma(p.r2a2, ur2, fma(ut, ut, fma(2.0 * ur, aup, up2s)));
   const double N = fma(R, P, -p.beta * ur2);                 // gamma^ij u_i u_j
-  const double G2 = (1.0 + N) * p.zp1;                       // (u^0)^2
-  const double iu0 = rsqrt(G2);
+  const double G2 = fma(N, p.zp1, p.zp1);                    // (u^0)^2 = (1+N)(1+z)
+  const double iu0 = rsqrt_nr(G2);
   const double u0 = G2 * iu0;
-  const double gur = fma(p.r2a2 * R - p.beta, ur, g.a * R * up);   // gamma^{rj} u_j
-  Xr = fma(gur, iu0, -p.beta);
-  Xt = R * ut * iu0;
-  Xp = R * fma(up, p.is2, g.a * ur) * iu0;
-  // derivatives: dz/dr = 2M (a^2 c^2 - r^2)/rho^4, dz/dth = 4 M r a^2 s c / rho^4
+  const double Riu0 = R * iu0;
+  // gamma^{rj} u_j / u^0 - beta
+  Xr = fma(fma(p.r2a2, ur, aup), Riu0, -p.beta * fma(ur, iu0, 1.0));
+  Xt = Riu0 * ut;
+  Xp = Riu0 * fma(up, p.is2, g.a * ur);
+  // derivatives: dz/dr = 2M (a^2 c^2 - r^2)/rho^4, dz/dth = 4 M r a^2 s c / rho^4; W = 1/(1+z)^2
   const double A = g.a2 * p.s * p.c;
-  const double W = p.h * p.h;
-  const double Wdzr = W * 2.0 * g.M * (g.a2 * p.c * p.c - p.r * p.r) * R2;
-  const double Wdzt = W * 4.0 * g.M * p.r * A * R2;
+  const double WR2 = p.h * p.h * R2 * g.twoM;
+  const double Wdzr = WR2 * fma(g.a2 * p.c, p.c, -p.r * p.r);
+  const double Wdzt = WR2 * 2.0 * p.r * A;
   const double lead = fma(0.5, u0, ur);                      // (u^0/2 + u_r)
   // (d_i gamma^jk) u_j u_k
-  const double quad_r = fma(-2.0 * p.r * R2, P, fma(2.0 * p.r * R, ur2, -Wdzr * ur2));
-  const double quad_t = fma(2.0 * A * R2, P, fma(-2.0 * R * p.c * p.is, up2s, -Wdzt * ur2));
+  const double twor = p.r + p.r;
+  const double quad_r = fma(-twor * R2, P, (twor * R - Wdzr) * ur2);
+  const double quad_t = fma(2.0 * A * R2, P, -fma(2.0 * R * p.c * p.is2 * p.s, up2s, Wdzt * ur2));
   const double hiu0 = 0.5 * iu0;
   Ur = fma(Wdzr, lead, -quad_r * hiu0);
   Ut = fma(Wdzt, lead, -quad_t * hiu0);
@@ -78,23 +122,23 @@ __device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double sgn
   const double g_rr = p.zp1, g_tt = p.rho2;
   const double g_rp = -g.a * s2 * p.zp1;
   const double g_pp = s2 * fma(g.a2 * s2, p.zp1, p.rho2);
-  const double alpha = sqrt(p.h);
+  const double alpha = p.h * rsqrt_nr(p.h);
   const double sqrtg = p.rho2 * p.s * p.zp1 * alpha;
-  const double gu_rr = p.r2a2 * p.R - p.beta, gu_tt = p.R, gu_pp = p.R * p.is2, gu_rp = g.a * p.R;
-  const double k = sgn * alpha * dt * 0.5;
+  const double gu_rr = fma(p.r2a2, p.R, -p.beta), gu_tt = p.R, gu_pp = p.R * p.is2, gu_rp = g.a * p.R;
+  const double hdt = sgn * dt * 0.5;
+  const double k = hdt * alpha;
   const double Dr = fma(g_rr, D[0], g_rp * D[2]), Dt = g_tt * D[1], Dp = fma(g_rp, D[0], g_pp * D[2]);
   const double mr = fma(k, Dr, ur), mt = fma(k, Dt, ut), mp = fma(k, Dp, up);   // u^-
-  const double N = fma(gu_rr * mr, mr, fma(gu_tt * mt, mt, fma(gu_pp * mp, mp, 2.0 * gu_rp * mr * mp)));
-  const double iu0 = alpha * rsqrt(1.0 + N);                                    // 1/ubar^0
-  const double f = sgn * dt * 0.5 * iu0;
+  double ar = fma(gu_rr, mr, gu_rp * mp), at = gu_tt * mt, ap = fma(gu_rp, mr, gu_pp * mp);
+  const double N = fma(ar, mr, fma(at, mt, ap * mp));
+  const double f = hdt * alpha * rsqrt_nr(1.0 + N);                             // q dt / (2 ubar^0)
   const double tr = f * B[0], tt = f * B[1], tp = f * B[2];                     // t^i
   // u~ = u^- + sqrtg eps (u^-)^j t^k
-  double ar = fma(gu_rr, mr, gu_rp * mp), at = gu_tt * mt, ap = fma(gu_rp, mr, gu_pp * mp);
   const double wr = fma(sqrtg, at * tp - ap * tt, mr);
   const double wt = fma(sqrtg, ap * tr - ar * tp, mt);
   const double wp = fma(sqrtg, ar * tt - at * tr, mp);
   const double t2 = fma(fma(g_rr, tr, g_rp * tp), tr, fma(g_tt * tt, tt, fma(g_rp, tr, g_pp * tp) * tp));
-  const double sc = 2.0 / (1.0 + t2);
+  const double sc = 2.0 * rcp_nr(1.0 + t2);
   const double sr = sc * tr, st = sc * tt, sp = sc * tp;
   ar = fma(gu_rr, wr, gu_rp * wp); at = gu_tt * wt; ap = fma(gu_rp, wr, gu_pp * wp);
   const double pr = fma(sqrtg, at * sp - ap * st, mr);                          // u^+
@@ -103,7 +147,7 @@ __device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double sgn
   ur = fma(k, Dr, pr); ut = fma(k, Dt, pt); up = fma(k, Dp, pp);
 }
 
-__device__ __forceinline__ double bilin(const double* __restrict__ F, size_t base, int pitch,
+__device__ __forceinline__ double bilin(const double* __restrict__ F, uint32_t base, int pitch,
                                         double wx, double wy) {
   const double f00 = __ldg(F + base), f10 = __ldg(F + base + 1);
   const double f01 = __ldg(F + base + pitch), f11 = __ldg(F + base + pitch + 1);
@@ -115,10 +159,27 @@ __device__ __forceinline__ void red_add(double* p, double v) {
   if (v != 0.0) atomicAdd(p, v);   // result unused -> RED.E.ADD.F64
 }
 
+// sin, cos of th0 + d from (s0, c0) for |d| <= 0.06 (angle addition, Taylor in d).
+__device__ __forceinline__ void sincos_shift(double s0, double c0, double d, double& s, double& c) {
+  const double d2 = d * d;
+  double ps = fma(d2, 1.0 / 362880.0, -1.0 / 5040.0);
+  ps = fma(ps, d2, 1.0 / 120.0);
+  ps = fma(ps, d2, -1.0 / 6.0);
+  const double sd = fma(ps * d2, d, d);                         // sin d
+  double pc = fma(d2, 1.0 / 3628800.0, -1.0 / 40320.0);
+  pc = fma(pc, d2, 1.0 / 720.0);
+  pc = fma(pc, d2, -1.0 / 24.0);
+  pc = fma(pc, d2, 0.5);
+  const double vd = pc * d2;                                    // 1 - cos d
+  s = s0 + fma(c0, sd, -s0 * vd);
+  c = c0 - fma(s0, sd, c0 * vd);
+}
+
 // General-window deposit (moves of more than one cell; never taken below the Courant limit).
-__device__ __noinline__ void deposit_far(const GridDev& g, double Q, double idt, double vphi,
+__device__ __noinline__ void deposit_far(const GridDev* gp, double Q, double idt, double vphi,
                                          double xa, double xb, double ya, double yb, double* Fr,
                                          double* Fth, double* Fph, uint32_t* status) {
+  const GridDev& g = *gp;
   const int ilo = (int)floor(fmin(xa, xb)), ihi = (int)floor(fmax(xa, xb)) + 1;
   const int jlo = (int)floor(fmin(ya, yb)), jhi = (int)floor(fmax(ya, yb)) + 1;
   if (status) atomicOr(status, GRPIC_STATUS_FAR_MOVE);
@@ -148,133 +209,235 @@ __device__ __noinline__ void deposit_far(const GridDev& g, double Q, double idt,
                       (1.0 / 6.0) * (S(xb - i) * S(ya - j) + S(xa - i) * S(yb - j))));
 }
 
-__device__ __forceinline__ void shape3(double d, double S[3]) {
-  // CIC weights of a point at offset d in [0,2) from the first of three consecutive nodes
-  S[0] = fmax(0.0, 1.0 - d);
-  S[1] = 1.0 - fabs(d - 1.0);
-  S[2] = fmax(0.0, d - 1.0);
+// Lane `lane` (< nslot) sums its slot over each run of equal window anchor, in particle order,
+// and adds the run total to F[anchor + off].  `runs` has bit q set where a run ends at lane q.
+__device__ __forceinline__ void reduce_runs(const double* st, bool owner, int lane, uint32_t runs,
+                                            uint32_t anchor, double* F, uint32_t off) {
+  const double* row = st + lane * kPad;
+  double acc = 0.0;
+#pragma unroll 8
+  for (int q = 0; q < 32; ++q) {
+    if (owner) acc += row[q];
+    if ((runs >> q) & 1u) {                                   // warp-uniform
+      const uint32_t b = __shfl_sync(kFull, anchor, q);
+      if (owner && acc != 0.0) atomicAdd(F + b + off, acc);
+      acc = 0.0;
+    }
+  }
 }
 
-__global__ void __launch_bounds__(128)
-push_deposit_kernel(GridDev g, grpic_particles ptc, grpic_fields f, grpic_current J, double dt,
-                    int K, uint32_t* status) {
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= ptc.n) return;
-  const uint32_t flag = ptc.flag[k];
-  if (flag & 2u) return;
-  const double x1 = ptc.x1[k], x2 = ptc.x2[k], x3 = ptc.x3[k];
-  double ur = ptc.u1[k], ut = ptc.u2[k], up = ptc.u3[k];
-  const double w = ptc.w[k];
-  const double sgn = (flag & 1u) ? 1.0 : -1.0;
+template <int MINB>
+__global__ void __launch_bounds__(kBlock, MINB)
+push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
+                    const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
+                    double dt, int K, uint32_t* status) {
+  __shared__ double stage_all[kBlock / 32][kSlotsA * kPad];
+  const int lane = threadIdx.x & 31;
+  double* st = stage_all[threadIdx.x >> 5];
+  const int64_t k = (int64_t)blockIdx.x * kBlock + threadIdx.x;
+  uint32_t flag = 2u;
+  if (k < ptc.n) flag = ptc.flag[k];
+  const bool active = !(flag & 2u);
+  if (!__any_sync(kFull, active)) return;
 
-  // ---- gather (first order, each component from its own staggered lattice) ----
-  const double xa = (x1 - g.xi_in) * g.inv_dxi, ya = x2 * g.inv_dth;
-  double D[3], B[3];
-  {
+  // deposit inputs; defaults describe "no contribution"
+  double Q = 0.0, vphi = 0.0, fx = 0.5, fy = 0.5, dx = 1.5, dy = 1.5;
+  uint32_t anchor = 0xFFFFFFFFu;
+  const double idt = 1.0 / dt;
+
+  if (active) {
+    const double x1 = ptc.x1[k], x2 = ptc.x2[k], x3 = ptc.x3[k];
+    double ur = ptc.u1[k], ut = ptc.u2[k], up = ptc.u3[k];
+    const double w = ptc.w[k];
+    const double sgn = (flag & 1u) ? 1.0 : -1.0;
+
+    // ---- gather (first order, each component from its own staggered lattice) ----
+    const double xa = (x1 - g.xi_in) * g.inv_dxi, ya = x2 * g.inv_dth;
     const double fin = floor(xa), fjn = floor(ya);
-    const double fih = floor(xa - 0.5), fjh = floor(ya - 0.5);
-    const int in = (int)fin, jn = (int)fjn, ih = (int)fih, jh = (int)fjh;
-    const double wxn = xa - fin, wyn = ya - fjn, wxh = xa - 0.5 - fih, wyh = ya - 0.5 - fjh;
-    D[0] = bilin(f.Dr, g.idx(ih, jn), g.pitch, wxh, wyn);
-    D[1] = bilin(f.Dth, g.idx(in, jh), g.pitch, wxn, wyh);
-    D[2] = bilin(f.Dph, g.idx(in, jn), g.pitch, wxn, wyn);
-    B[0] = bilin(f.Br, g.idx(in, jh), g.pitch, wxn, wyh);
-    B[1] = bilin(f.Bth, g.idx(ih, jn), g.pitch, wxh, wyn);
-    B[2] = bilin(f.Bph, g.idx(ih, jh), g.pitch, wxh, wyh);
-  }
-
-  // ---- Boris (full dt) at x^n ----
-  const double r0 = exp(x1);
-  double s, c;
-  sincos(x2, &s, &c);
-  const Pos p0 = make_pos(g, r0, s, c);
-  boris(g, p0, sgn, dt, D, B, ur, ut, up);
-
-  // ---- geodesic predictor + K correctors (Eq.14, 15) ----
-  double Xr0, Xt0, Xp0, Ur0, Ut0;
-  geodesic_rhs(g, p0, ur, ut, up, Xr0, Xt0, Xp0, Ur0, Ut0);
-  double r = fma(Xr0, dt, r0), th = fma(Xt0, dt, x2), ph = fma(Xp0, dt, x3);
-  double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
-  const double hdt = 0.5 * dt;
-  for (int it = 0; it < K; ++it) {
-    sincos(th, &s, &c);
-    const Pos p1 = make_pos(g, r, s, c);
-    double Xr, Xt, Xp, Ur, Ut;
-    geodesic_rhs(g, p1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
-    r = fma(hdt, Xr + Xr0, r0);
-    th = fma(hdt, Xt + Xt0, x2);
-    ph = fma(hdt, Xp + Xp0, x3);
-    vr = fma(hdt, Ur + Ur0, ur);
-    vt = fma(hdt, Ut + Ut0, ut);
-  }
-
-  // ---- new logical position, reflection, removal ----
-  const double x1n = log(r);
-  const double th_dep = th;
-  if (th < 0.0) { th = -th; vt = -vt; }
-  if (th > M_PI) { th = 2.0 * M_PI - th; vt = -vt; }
-  uint32_t nflag = flag, ncell;
-  const bool finite = isfinite(x1n) && isfinite(th) && isfinite(ph) && isfinite(vr) && isfinite(vt);
-  const bool out = !finite || (x1n < g.xi_in) || (x1n >= g.xi_out);
-  if (out) {
-    nflag |= 2u;
-    ncell = 0xFFFFFFFFu;
-    if (!finite && status) atomicOr(status, GRPIC_STATUS_NONFINITE);
-  } else {
-    int ic = (int)floor((x1n - g.xi_in) / g.dxi);
-    int jc = (int)floor(th / g.dth);
-    ic = min(max(ic, 0), g.nr - 1);
-    jc = min(max(jc, 0), g.nth - 1);
-    ncell = (uint32_t)(jc * g.nr + ic);
-  }
-  ptc.x1[k] = x1n; ptc.x2[k] = th; ptc.x3[k] = ph;
-  ptc.u1[k] = vr; ptc.u2[k] = vt; ptc.u3[k] = up;
-  ptc.cell[k] = ncell;
-  ptc.flag[k] = nflag;
-  if (!finite) return;
-
-  // ---- charge-conserving deposit of the move (Eq.21-23) ----
-  const double xb = (x1n - g.xi_in) * g.inv_dxi, yb = th_dep * g.inv_dth;
-  const double Q = sgn * w, idt = 1.0 / dt;
-  const double vphi = Q * (ph - x3) * idt;
-  const int ia = (int)floor(xa), ib = (int)floor(xb), ja = (int)floor(ya), jb = (int)floor(yb);
-  const int i0 = min(ia, ib), j0 = min(ja, jb);
-  if (max(ia, ib) - i0 > 1 || max(ja, jb) - j0 > 1) {
-    deposit_far(g, Q, idt, vphi, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
-    return;
-  }
-  if (i0 < -g.ng || i0 + 2 > g.nr + g.ng || j0 < -g.ng || j0 + 2 > g.nth + g.ng) {
-    if (status) atomicOr(status, GRPIC_STATUS_OFFGRID);
-    return;
-  }
-  double Sa[3], Sb[3], Ta[3], Tb[3];
-  shape3(xa - i0, Sa); shape3(xb - i0, Sb); shape3(ya - j0, Ta); shape3(yb - j0, Tb);
-  const size_t base = g.idx(i0, j0);
-  const double hq = -0.5 * Q * idt;
-#pragma unroll
-  for (int j = 0; j < 3; ++j) {
-    const double at = hq * (Tb[j] + Ta[j]);
-    const double f0 = at * (Sb[0] - Sa[0]);                 // F_r(i0+1/2, j0+j)
-    const double f1 = fma(at, Sb[1] - Sa[1], f0);           // F_r(i0+3/2, j0+j)
-    red_add(J.Fr + base + (size_t)j * g.pitch, f0);
-    red_add(J.Fr + base + (size_t)j * g.pitch + 1, f1);
-  }
-#pragma unroll
-  for (int i = 0; i < 3; ++i) {
-    const double as = hq * (Sb[i] + Sa[i]);
-    const double f0 = as * (Tb[0] - Ta[0]);                 // F_th(i0+i, j0+1/2)
-    const double f1 = fma(as, Tb[1] - Ta[1], f0);           // F_th(i0+i, j0+3/2)
-    red_add(J.Fth + base + i, f0);
-    red_add(J.Fth + base + g.pitch + i, f1);
-  }
-#pragma unroll
-  for (int j = 0; j < 3; ++j)
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      const double sh = (1.0 / 3.0) * fma(Sb[i], Tb[j], Sa[i] * Ta[j]) +
-                        (1.0 / 6.0) * fma(Sb[i], Ta[j], Sa[i] * Tb[j]);
-      red_add(J.Fph + base + (size_t)j * g.pitch + i, vphi * sh);
+    const int ia = (int)fin, ja = (int)fjn;
+    double D[3], B[3];
+    {
+      const double fih = floor(xa - 0.5), fjh = floor(ya - 0.5);
+      const int ih = (int)fih, jh = (int)fjh;
+      const double wxn = xa - fin, wyn = ya - fjn, wxh = xa - 0.5 - fih, wyh = ya - 0.5 - fjh;
+      const uint32_t bnn = (uint32_t)g.idx(ia, ja), bhn = (uint32_t)g.idx(ih, ja);
+      const uint32_t bnh = (uint32_t)g.idx(ia, jh), bhh = (uint32_t)g.idx(ih, jh);
+      D[0] = bilin(f.Dr, bhn, g.pitch, wxh, wyn);
+      D[1] = bilin(f.Dth, bnh, g.pitch, wxn, wyh);
+      D[2] = bilin(f.Dph, bnn, g.pitch, wxn, wyn);
+      B[0] = bilin(f.Br, bnh, g.pitch, wxn, wyh);
+      B[1] = bilin(f.Bth, bhn, g.pitch, wxh, wyn);
+      B[2] = bilin(f.Bph, bhh, g.pitch, wxh, wyh);
     }
+
+    // ---- Boris (full dt) at x^n ----
+    const double r0 = exp(x1);
+    double s0, c0;
+    sincos(x2, &s0, &c0);
+    const Pos p0 = make_pos(g, r0, s0, c0);
+    boris(g, p0, sgn, dt, D, B, ur, ut, up);
+
+    // ---- geodesic predictor + K correctors (Eq.14, 15) ----
+    double Xr0, Xt0, Xp0, Ur0, Ut0;
+    geodesic_rhs(g, p0, ur, ut, up, Xr0, Xt0, Xp0, Ur0, Ut0);
+    double dr = Xr0 * dt, dth = Xt0 * dt, dph = Xp0 * dt;      // increments from x^n
+    double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
+    const double hdt = 0.5 * dt;
+    for (int it = 0; it < K; ++it) {
+      double s, c;
+      if (fabs(dth) <= 0.06) sincos_shift(s0, c0, dth, s, c);
+      else sincos(x2 + dth, &s, &c);
+      const Pos p1 = make_pos(g, r0 + dr, s, c);
+      double Xr, Xt, Xp, Ur, Ut;
+      geodesic_rhs(g, p1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
+      dr = hdt * (Xr + Xr0);
+      dth = hdt * (Xt + Xt0);
+      dph = hdt * (Xp + Xp0);
+      vr = fma(hdt, Ur + Ur0, ur);
+      vt = fma(hdt, Ut + Ut0, ut);
+    }
+    const double r = r0 + dr, ph = x3 + dph;
+    double th = x2 + dth;
+
+    // ---- new logical position: ln r = x1 + 2 atanh(dr / (2 r0 + dr)) ----
+    double x1n;
+    {
+      const double wq = dr * rcp_nr(r0 + r);
+      if (fabs(wq) <= 0.03) {
+        const double w2 = wq * wq;
+        double pl = fma(w2, 1.0 / 11.0, 1.0 / 9.0);
+        pl = fma(pl, w2, 1.0 / 7.0);
+        pl = fma(pl, w2, 1.0 / 5.0);
+        pl = fma(pl, w2, 1.0 / 3.0);
+        const double at = fma(pl * w2, wq, wq);
+        x1n = fma(2.0, at, x1);
+      } else {
+        x1n = log(r);
+      }
+    }
+    // ---- reflection, removal, new cell ----
+    const double th_dep = th;
+    if (th < 0.0) { th = -th; vt = -vt; }
+    if (th > M_PI) { th = 2.0 * M_PI - th; vt = -vt; }
+    const double xb = (x1n - g.xi_in) * g.inv_dxi, yb = th_dep * g.inv_dth;
+    uint32_t nflag = flag, ncell;
+    const bool finite = isfinite(x1n) && isfinite(th) && isfinite(ph) && isfinite(vr) && isfinite(vt);
+    const bool out = !finite || (x1n < g.xi_in) || (x1n >= g.xi_out);
+    if (out) {
+      nflag |= 2u;
+      ncell = 0xFFFFFFFFu;
+      if (!finite && status) atomicOr(status, GRPIC_STATUS_NONFINITE);
+    } else {
+      // cell = floor of the quotient; the product form decides unless it is within 1e-7 of
+      // a cell edge, where the quotient itself is taken (same decision as a division)
+      double cx = xb, cy = th * g.inv_dth;
+      if (fabs(cx - rint(cx)) < 1e-7) cx = (x1n - g.xi_in) / g.dxi;
+      if (fabs(cy - rint(cy)) < 1e-7) cy = th / g.dth;
+      int ic = (int)floor(cx), jc = (int)floor(cy);
+      ic = min(max(ic, 0), g.nr - 1);
+      jc = min(max(jc, 0), g.nth - 1);
+      ncell = (uint32_t)(jc * g.nr + ic);
+    }
+    ptc.x1[k] = x1n; ptc.x2[k] = th; ptc.x3[k] = ph;
+    ptc.u1[k] = vr; ptc.u2[k] = vt; ptc.u3[k] = up;
+    ptc.cell[k] = ncell;
+    ptc.flag[k] = nflag;
+
+    // ---- deposit set-up: window anchored at (ia-1, ja-1) ----
+    if (finite) {
+      const double q = sgn * w;
+      const double vph = q * dph * idt;
+      const double ddx = xb - (double)(ia - 1), ddy = yb - (double)(ja - 1);   // in [0,3) if near
+      const bool near = (ddx >= 0.0) && (ddx < 3.0) && (ddy >= 0.0) && (ddy < 3.0);
+      const bool ingrid = (ia - 1 >= -g.ng) && (ia + 2 <= g.nr + g.ng) && (ja - 1 >= -g.ng) &&
+                          (ja + 2 <= g.nth + g.ng);
+      if (near && ingrid) {
+        Q = q; vphi = vph; fx = xa - fin; fy = ya - fjn; dx = ddx; dy = ddy;
+        anchor = (uint32_t)g.idx(ia - 1, ja - 1);
+      } else {
+        deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
+      }
+    }
+  }
+
+  // ---- charge-conserving deposit of the move (Eq.21-23), warp-cooperative ----
+  // shapes on the 4 window nodes: old position (cell-relative fx in [0,1)), new position d in [0,3)
+  const double Sa1 = 1.0 - fx, Sa2 = fx, Ta1 = 1.0 - fy, Ta2 = fy;
+  double Sb[4], Tb[4];
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    Sb[m] = fmax(0.0, 1.0 - fabs(dx - (double)m));
+    Tb[m] = fmax(0.0, 1.0 - fabs(dy - (double)m));
+  }
+  const uint32_t nxt = __shfl_down_sync(kFull, anchor, 1);
+  const uint32_t runs = __ballot_sync(kFull, (lane == 31) || (nxt != anchor));
+  const bool direct = __popc(runs) > kDirectRuns;
+  const double hq = -0.5 * Q * idt;
+  // prefix sums of the shape differences (Eq.21): faces 0..2 of the window
+  const double Px0 = Sb[0], Px1 = Px0 + (Sb[1] - Sa1), Px2 = Px1 + (Sb[2] - Sa2);
+  const double Py0 = Tb[0], Py1 = Py0 + (Tb[1] - Ta1), Py2 = Py1 + (Tb[2] - Ta2);
+  const double Ay[4] = {hq * Tb[0], hq * (Tb[1] + Ta1), hq * (Tb[2] + Ta2), hq * Tb[3]};
+  const double Ax[4] = {hq * Sb[0], hq * (Sb[1] + Sa1), hq * (Sb[2] + Sa2), hq * Sb[3]};
+  const double Px[3] = {Px0, Px1, Px2}, Py[3] = {Py0, Py1, Py2};
+  // F_phi (Eq.23): Sb_i U_j + Sa_i V_j
+  double U[4], V[4];
+  {
+    const double c3 = vphi * (1.0 / 3.0), c6 = vphi * (1.0 / 6.0);
+    U[0] = c3 * Tb[0]; U[3] = c3 * Tb[3];
+    U[1] = fma(c3, Tb[1], c6 * Ta1); U[2] = fma(c3, Tb[2], c6 * Ta2);
+    V[0] = c6 * Tb[0]; V[3] = c6 * Tb[3];
+    V[1] = fma(c3, Ta1, c6 * Tb[1]); V[2] = fma(c3, Ta2, c6 * Tb[2]);
+  }
+  const uint32_t pitch = (uint32_t)g.pitch;
+  if (direct) {
+    if (anchor != 0xFFFFFFFFu) {
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int m = 0; m < 3; ++m) red_add(J.Fr + anchor + j * pitch + m, Ay[j] * Px[m]);
+#pragma unroll
+      for (int m = 0; m < 3; ++m)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) red_add(J.Fth + anchor + m * pitch + i, Ax[i] * Py[m]);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        red_add(J.Fph + anchor + j * pitch + 0, Sb[0] * U[j]);
+        red_add(J.Fph + anchor + j * pitch + 1, fma(Sb[1], U[j], Sa1 * V[j]));
+        red_add(J.Fph + anchor + j * pitch + 2, fma(Sb[2], U[j], Sa2 * V[j]));
+        red_add(J.Fph + anchor + j * pitch + 3, Sb[3] * U[j]);
+      }
+    }
+    return;
+  }
+  // phase A: slots 0..11 = F_r (row j, face m), 12..23 = F_theta (face m, column i)
+#pragma unroll
+  for (int j = 0; j < 4; ++j)
+#pragma unroll
+    for (int m = 0; m < 3; ++m) st[(j * 3 + m) * kPad + lane] = Ay[j] * Px[m];
+#pragma unroll
+  for (int m = 0; m < 3; ++m)
+#pragma unroll
+    for (int i = 0; i < 4; ++i) st[(12 + m * 4 + i) * kPad + lane] = Ax[i] * Py[m];
+  __syncwarp();
+  {
+    const bool isr = lane < 12;
+    const int l2 = isr ? lane : lane - 12;
+    const uint32_t off = isr ? (uint32_t)(l2 / 3) * pitch + (uint32_t)(l2 % 3)
+                             : (uint32_t)(l2 / 4) * pitch + (uint32_t)(l2 % 4);
+    reduce_runs(st, lane < kSlotsA, lane, runs, anchor, isr ? J.Fr : J.Fth, off);
+  }
+  __syncwarp();
+  // phase B: slots 0..15 = F_phi (row j, column i)
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    st[(j * 4 + 0) * kPad + lane] = Sb[0] * U[j];
+    st[(j * 4 + 1) * kPad + lane] = fma(Sb[1], U[j], Sa1 * V[j]);
+    st[(j * 4 + 2) * kPad + lane] = fma(Sb[2], U[j], Sa2 * V[j]);
+    st[(j * 4 + 3) * kPad + lane] = Sb[3] * U[j];
+  }
+  __syncwarp();
+  reduce_runs(st, lane < kSlotsB, lane, runs, anchor, J.Fph,
+              (uint32_t)(lane >> 2) * pitch + (uint32_t)(lane & 3));
 }
 
 }  // namespace
@@ -289,10 +452,9 @@ extern "C" int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const gr
       !flux->Fr || !flux->Fth || !flux->Fph)
     return GRPIC_ERR_ARG;
   if (ptc->n == 0) return GRPIC_OK;
-  const int block = 128;
-  const int64_t grid = (ptc->n + block - 1) / block;
+  const int64_t grid = (ptc->n + kBlock - 1) / kBlock;
   if (grid > 0x7FFFFFFFLL) return GRPIC_ERR_ARG;
-  push_deposit_kernel<<<(unsigned)grid, block, 0, (cudaStream_t)stream>>>(
+  push_deposit_kernel<4><<<(unsigned)grid, kBlock, 0, (cudaStream_t)stream>>>(
       ctx->g, *ptc, *fields, *flux, dt, ctx->p.geo_iters, status);
   grpic_count_launches(1);
   return grpic_launch_ok();
