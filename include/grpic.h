@@ -105,7 +105,8 @@ int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes);
  * F_ph = J^ph dV  of the step are ACCUMULATED (+=) into `flux` (zero it first; guards and
  * theta ghost rows receive the parts deposited beyond the domain).  `fields` must have
  * valid guard / ghost values (grpic_field_step and grpic_fill_guards maintain them).
- * `status` may be NULL. */
+ * `status` may be NULL.  The particle arrays must be 16-byte aligned (they are streamed
+ * through shared memory with bulk TMA copies); otherwise GRPIC_ERR_ARG. */
 int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                        grpic_current* flux, double dt, uint32_t* status, void* stream);
 

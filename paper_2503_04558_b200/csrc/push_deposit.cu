@@ -13,18 +13,20 @@
 // 4x4 node window anchored one node below its OLD cell (12 F_r faces, 12 F_theta faces, 16
 // F_phi nodes).  Particles are cell-sorted, so the lanes of a warp form a few runs of equal
 // window anchor.  Each warp transposes its 32 x 40 contributions through a private
-// shared-memory tile (slot-major, padded to 33), lane L then sums slot L over each run in
-// particle order and issues ONE red.global.add.f64 per (run, slot).  Warps with many runs
-// (unsorted or very sparse input) fall back to per-lane reductions of their non-zero values.
+// shared-memory tile (slot-major, padded to 33) in two halves of 20 slots; lane L then sums
+// five slots over four consecutive particles, run by run, and issues one red.global.add.f64
+// per (run piece, slot): 10 warp-wide RED instructions with 8-way address sharing instead of
+// 21-40 with 32-way sharing.  Warps with many runs (unsorted or very sparse input) fall back to per-lane
+// reductions of their non-zero values.
 #include <math.h>
+#include <stdlib.h>
 
 #include "grpic_internal.cuh"
 
 namespace {
 
 constexpr int kBlock = 128;
-constexpr int kSlotsA = 24;          // phase A: 12 F_r + 12 F_theta slots
-constexpr int kSlotsB = 16;          // phase B: 16 F_phi slots
+constexpr int kSlots = 40;           // 12 F_r + 12 F_theta + 16 F_phi slots of the 4x4 window
 constexpr int kPad = 33;             // particles per slot row (+1 against bank conflicts)
 constexpr unsigned kFull = 0xffffffffu;
 constexpr int kDirectRuns = 12;      // more runs than this in a warp: per-lane reductions
@@ -147,14 +149,6 @@ __device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double sgn
   ur = fma(k, Dr, pr); ut = fma(k, Dt, pt); up = fma(k, Dp, pp);
 }
 
-__device__ __forceinline__ double bilin(const double* __restrict__ F, uint32_t base, int pitch,
-                                        double wx, double wy) {
-  const double f00 = __ldg(F + base), f10 = __ldg(F + base + 1);
-  const double f01 = __ldg(F + base + pitch), f11 = __ldg(F + base + pitch + 1);
-  const double lo = fma(wx, f10 - f00, f00), hi = fma(wx, f11 - f01, f01);
-  return fma(wy, hi - lo, lo);
-}
-
 __device__ __forceinline__ void red_add(double* p, double v) {
   if (v != 0.0) atomicAdd(p, v);   // result unused -> RED.E.ADD.F64
 }
@@ -209,158 +203,45 @@ __device__ __noinline__ void deposit_far(const GridDev* gp, double Q, double idt
                       (1.0 / 6.0) * (S(xb - i) * S(ya - j) + S(xa - i) * S(yb - j))));
 }
 
-// Lane `lane` (< nslot) sums its slot over each run of equal window anchor, in particle order,
-// and adds the run total to F[anchor + off].  `runs` has bit q set where a run ends at lane q.
-__device__ __forceinline__ void reduce_runs(const double* st, bool owner, int lane, uint32_t runs,
-                                            uint32_t anchor, double* F, uint32_t off) {
-  const double* row = st + lane * kPad;
-  double acc = 0.0;
-#pragma unroll 8
-  for (int q = 0; q < 32; ++q) {
-    if (owner) acc += row[q];
-    if ((runs >> q) & 1u) {                                   // warp-uniform
-      const uint32_t b = __shfl_sync(kFull, anchor, q);
-      if (owner && acc != 0.0) atomicAdd(F + b + off, acc);
-      acc = 0.0;
+// Run reduction of one staged 20 x 32 half-tile (phase ph = slots 20*ph .. 20*ph+19).  Lane L
+// owns the five slots 5*(L&3)..+4 of the phase for the four particles 4*(L>>2)..+3: it sums
+// them in particle order in five independent accumulators and adds the partial sums to
+// F[anchor + off] wherever a run of equal window anchor ends inside its range (and at the end
+// of the range).  `ends` = run ends | 0x88888888.
+__device__ __forceinline__ void reduce_runs(const double* st, int lane, uint32_t ends,
+                                            uint32_t anchor, double* const F[5]) {
+  const int p0 = (lane >> 2) * 4;
+  const double* row = st + (lane & 3) * 5 * kPad + p0;
+  const uint32_t mine = ends >> p0;
+  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+#pragma unroll
+  for (int q = 0; q < 4; ++q) {
+    const uint32_t b = __shfl_sync(kFull, anchor, p0 + q);
+#pragma unroll
+    for (int m = 0; m < 5; ++m) acc[m] += row[m * kPad + q];
+    if ((mine >> q) & 1u) {
+#pragma unroll
+      for (int m = 0; m < 5; ++m) {
+        if (acc[m] != 0.0) atomicAdd(F[m] + b, acc[m]);
+        acc[m] = 0.0;
+      }
     }
   }
 }
 
-template <int MINB>
-__global__ void __launch_bounds__(kBlock, MINB)
-push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
-                    const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
-                    double dt, int K, uint32_t* status) {
-  __shared__ double stage_all[kBlock / 32][kSlotsA * kPad];
-  const int lane = threadIdx.x & 31;
-  double* st = stage_all[threadIdx.x >> 5];
-  const int64_t k = (int64_t)blockIdx.x * kBlock + threadIdx.x;
-  uint32_t flag = 2u;
-  if (k < ptc.n) flag = ptc.flag[k];
-  const bool active = !(flag & 2u);
-  if (!__any_sync(kFull, active)) return;
+// global array + in-window offset of deposit slot t (0..11 F_r, 12..23 F_theta, 24..39 F_phi)
+__device__ __forceinline__ double* slot_target(const grpic_current& J, int t, uint32_t pitch) {
+  if (t < 12) return J.Fr + (uint32_t)(t / 3) * pitch + (uint32_t)(t % 3);
+  if (t < 24) return J.Fth + (uint32_t)((t - 12) / 4) * pitch + (uint32_t)((t - 12) % 4);
+  return J.Fph + (uint32_t)((t - 24) / 4) * pitch + (uint32_t)((t - 24) % 4);
+}
 
-  // deposit inputs; defaults describe "no contribution"
-  double Q = 0.0, vphi = 0.0, fx = 0.5, fy = 0.5, dx = 1.5, dy = 1.5;
-  uint32_t anchor = 0xFFFFFFFFu;
-  const double idt = 1.0 / dt;
-
-  if (active) {
-    const double x1 = ptc.x1[k], x2 = ptc.x2[k], x3 = ptc.x3[k];
-    double ur = ptc.u1[k], ut = ptc.u2[k], up = ptc.u3[k];
-    const double w = ptc.w[k];
-    const double sgn = (flag & 1u) ? 1.0 : -1.0;
-
-    // ---- gather (first order, each component from its own staggered lattice) ----
-    const double xa = (x1 - g.xi_in) * g.inv_dxi, ya = x2 * g.inv_dth;
-    const double fin = floor(xa), fjn = floor(ya);
-    const int ia = (int)fin, ja = (int)fjn;
-    double D[3], B[3];
-    {
-      const double fih = floor(xa - 0.5), fjh = floor(ya - 0.5);
-      const int ih = (int)fih, jh = (int)fjh;
-      const double wxn = xa - fin, wyn = ya - fjn, wxh = xa - 0.5 - fih, wyh = ya - 0.5 - fjh;
-      const uint32_t bnn = (uint32_t)g.idx(ia, ja), bhn = (uint32_t)g.idx(ih, ja);
-      const uint32_t bnh = (uint32_t)g.idx(ia, jh), bhh = (uint32_t)g.idx(ih, jh);
-      D[0] = bilin(f.Dr, bhn, g.pitch, wxh, wyn);
-      D[1] = bilin(f.Dth, bnh, g.pitch, wxn, wyh);
-      D[2] = bilin(f.Dph, bnn, g.pitch, wxn, wyn);
-      B[0] = bilin(f.Br, bnh, g.pitch, wxn, wyh);
-      B[1] = bilin(f.Bth, bhn, g.pitch, wxh, wyn);
-      B[2] = bilin(f.Bph, bhh, g.pitch, wxh, wyh);
-    }
-
-    // ---- Boris (full dt) at x^n ----
-    const double r0 = exp(x1);
-    double s0, c0;
-    sincos(x2, &s0, &c0);
-    const Pos p0 = make_pos(g, r0, s0, c0);
-    boris(g, p0, sgn, dt, D, B, ur, ut, up);
-
-    // ---- geodesic predictor + K correctors (Eq.14, 15) ----
-    double Xr0, Xt0, Xp0, Ur0, Ut0;
-    geodesic_rhs(g, p0, ur, ut, up, Xr0, Xt0, Xp0, Ur0, Ut0);
-    double dr = Xr0 * dt, dth = Xt0 * dt, dph = Xp0 * dt;      // increments from x^n
-    double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
-    const double hdt = 0.5 * dt;
-    for (int it = 0; it < K; ++it) {
-      double s, c;
-      if (fabs(dth) <= 0.06) sincos_shift(s0, c0, dth, s, c);
-      else sincos(x2 + dth, &s, &c);
-      const Pos p1 = make_pos(g, r0 + dr, s, c);
-      double Xr, Xt, Xp, Ur, Ut;
-      geodesic_rhs(g, p1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
-      dr = hdt * (Xr + Xr0);
-      dth = hdt * (Xt + Xt0);
-      dph = hdt * (Xp + Xp0);
-      vr = fma(hdt, Ur + Ur0, ur);
-      vt = fma(hdt, Ut + Ut0, ut);
-    }
-    const double r = r0 + dr, ph = x3 + dph;
-    double th = x2 + dth;
-
-    // ---- new logical position: ln r = x1 + 2 atanh(dr / (2 r0 + dr)) ----
-    double x1n;
-    {
-      const double wq = dr * rcp_nr(r0 + r);
-      if (fabs(wq) <= 0.03) {
-        const double w2 = wq * wq;
-        double pl = fma(w2, 1.0 / 11.0, 1.0 / 9.0);
-        pl = fma(pl, w2, 1.0 / 7.0);
-        pl = fma(pl, w2, 1.0 / 5.0);
-        pl = fma(pl, w2, 1.0 / 3.0);
-        const double at = fma(pl * w2, wq, wq);
-        x1n = fma(2.0, at, x1);
-      } else {
-        x1n = log(r);
-      }
-    }
-    // ---- reflection, removal, new cell ----
-    const double th_dep = th;
-    if (th < 0.0) { th = -th; vt = -vt; }
-    if (th > M_PI) { th = 2.0 * M_PI - th; vt = -vt; }
-    const double xb = (x1n - g.xi_in) * g.inv_dxi, yb = th_dep * g.inv_dth;
-    uint32_t nflag = flag, ncell;
-    const bool finite = isfinite(x1n) && isfinite(th) && isfinite(ph) && isfinite(vr) && isfinite(vt);
-    const bool out = !finite || (x1n < g.xi_in) || (x1n >= g.xi_out);
-    if (out) {
-      nflag |= 2u;
-      ncell = 0xFFFFFFFFu;
-      if (!finite && status) atomicOr(status, GRPIC_STATUS_NONFINITE);
-    } else {
-      // cell = floor of the quotient; the product form decides unless it is within 1e-7 of
-      // a cell edge, where the quotient itself is taken (same decision as a division)
-      double cx = xb, cy = th * g.inv_dth;
-      if (fabs(cx - rint(cx)) < 1e-7) cx = (x1n - g.xi_in) / g.dxi;
-      if (fabs(cy - rint(cy)) < 1e-7) cy = th / g.dth;
-      int ic = (int)floor(cx), jc = (int)floor(cy);
-      ic = min(max(ic, 0), g.nr - 1);
-      jc = min(max(jc, 0), g.nth - 1);
-      ncell = (uint32_t)(jc * g.nr + ic);
-    }
-    ptc.x1[k] = x1n; ptc.x2[k] = th; ptc.x3[k] = ph;
-    ptc.u1[k] = vr; ptc.u2[k] = vt; ptc.u3[k] = up;
-    ptc.cell[k] = ncell;
-    ptc.flag[k] = nflag;
-
-    // ---- deposit set-up: window anchored at (ia-1, ja-1) ----
-    if (finite) {
-      const double q = sgn * w;
-      const double vph = q * dph * idt;
-      const double ddx = xb - (double)(ia - 1), ddy = yb - (double)(ja - 1);   // in [0,3) if near
-      const bool near = (ddx >= 0.0) && (ddx < 3.0) && (ddy >= 0.0) && (ddy < 3.0);
-      const bool ingrid = (ia - 1 >= -g.ng) && (ia + 2 <= g.nr + g.ng) && (ja - 1 >= -g.ng) &&
-                          (ja + 2 <= g.nth + g.ng);
-      if (near && ingrid) {
-        Q = q; vphi = vph; fx = xa - fin; fy = ya - fjn; dx = ddx; dy = ddy;
-        anchor = (uint32_t)g.idx(ia - 1, ja - 1);
-      } else {
-        deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
-      }
-    }
-  }
-
-  // ---- charge-conserving deposit of the move (Eq.21-23), warp-cooperative ----
+// Warp-cooperative charge-conserving deposit of 32 moves (Eq.21-23).  Per lane: charge Q,
+// azimuthal flux Q dphi/dt, old in-cell offsets (fx, fy) in [0,1), new window offsets (dx, dy)
+// in [0,3), window anchor index (0xFFFFFFFF = nothing to deposit; then Q = vphi = 0).
+__device__ __forceinline__ void deposit_warp(const GridDev& g, const grpic_current& J, double* st,
+                                             int lane, double Q, double vphi, double fx, double fy,
+                                             double dx, double dy, uint32_t anchor, double idt) {
   // shapes on the 4 window nodes: old position (cell-relative fx in [0,1)), new position d in [0,3)
   const double Sa1 = 1.0 - fx, Sa2 = fx, Ta1 = 1.0 - fy, Ta2 = fy;
   double Sb[4], Tb[4];
@@ -409,35 +290,291 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     }
     return;
   }
-  // phase A: slots 0..11 = F_r (row j, face m), 12..23 = F_theta (face m, column i)
+  // slots 0..11 = F_r (row j, face m), 12..23 = F_theta (face m, column i), 24..39 = F_phi;
+  // staged and reduced in two halves of 20 slots
 #pragma unroll
   for (int j = 0; j < 4; ++j)
 #pragma unroll
     for (int m = 0; m < 3; ++m) st[(j * 3 + m) * kPad + lane] = Ay[j] * Px[m];
 #pragma unroll
-  for (int m = 0; m < 3; ++m)
+  for (int m = 0; m < 2; ++m)
 #pragma unroll
     for (int i = 0; i < 4; ++i) st[(12 + m * 4 + i) * kPad + lane] = Ax[i] * Py[m];
   __syncwarp();
-  {
-    const bool isr = lane < 12;
-    const int l2 = isr ? lane : lane - 12;
-    const uint32_t off = isr ? (uint32_t)(l2 / 3) * pitch + (uint32_t)(l2 % 3)
-                             : (uint32_t)(l2 / 4) * pitch + (uint32_t)(l2 % 4);
-    reduce_runs(st, lane < kSlotsA, lane, runs, anchor, isr ? J.Fr : J.Fth, off);
-  }
+  const uint32_t ends = runs | 0x88888888u;
+  double* F[5];
+#pragma unroll
+  for (int m = 0; m < 5; ++m) F[m] = slot_target(J, (lane & 3) * 5 + m, pitch);
+  reduce_runs(st, lane, ends, anchor, F);
   __syncwarp();
-  // phase B: slots 0..15 = F_phi (row j, column i)
+#pragma unroll
+  for (int i = 0; i < 4; ++i) st[i * kPad + lane] = Ax[i] * Py[2];
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    st[(j * 4 + 0) * kPad + lane] = Sb[0] * U[j];
-    st[(j * 4 + 1) * kPad + lane] = fma(Sb[1], U[j], Sa1 * V[j]);
-    st[(j * 4 + 2) * kPad + lane] = fma(Sb[2], U[j], Sa2 * V[j]);
-    st[(j * 4 + 3) * kPad + lane] = Sb[3] * U[j];
+    st[(4 + j * 4 + 0) * kPad + lane] = Sb[0] * U[j];
+    st[(4 + j * 4 + 1) * kPad + lane] = fma(Sb[1], U[j], Sa1 * V[j]);
+    st[(4 + j * 4 + 2) * kPad + lane] = fma(Sb[2], U[j], Sa2 * V[j]);
+    st[(4 + j * 4 + 3) * kPad + lane] = Sb[3] * U[j];
   }
   __syncwarp();
-  reduce_runs(st, lane < kSlotsB, lane, runs, anchor, J.Fph,
-              (uint32_t)(lane >> 2) * pitch + (uint32_t)(lane & 3));
+#pragma unroll
+  for (int m = 0; m < 5; ++m) F[m] = slot_target(J, 20 + (lane & 3) * 5 + m, pitch);
+  reduce_runs(st, lane, ends, anchor, F);
+}
+
+// ---- TMA (cp.async.bulk) + mbarrier plumbing for the double-buffered particle tiles ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
+}
+
+// One tile of particle input staged in shared memory (structure of arrays, 128 particles).
+struct __align__(128) PtcTile {
+  double x1[kBlock], x2[kBlock], x3[kBlock], u1[kBlock], u2[kBlock], u3[kBlock], w[kBlock];
+  uint32_t flag[kBlock];
+};
+constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
+
+// Persistent kernel: each CTA walks the 128-particle tiles blockIdx.x, +gridDim.x, ...; the
+// particle state of the NEXT tile is fetched by eight 1-D bulk TMA copies into the other
+// shared-memory stage while the current tile is pushed, so no warp waits on a DRAM round trip
+// for its particle.  The last, partial tile (n % 128 != 0) is staged with plain loads.
+template <int MINB>
+__global__ void __launch_bounds__(kBlock, MINB)
+push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
+                    const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
+                    double dt, int K, uint32_t* status) {
+  __shared__ PtcTile tiles[2];
+  __shared__ __align__(8) uint64_t full[2];
+  __shared__ double stage_all[kBlock / 32][(kSlots / 2) * kPad];
+  const int tid = threadIdx.x, lane = tid & 31;
+  double* st = stage_all[tid >> 5];
+  const int64_t ntiles = (ptc.n + kBlock - 1) / kBlock;
+  const double idt = 1.0 / dt;
+
+  auto issue = [&](int64_t tile, int stage) {       // thread 0 only; full tiles only
+    const int64_t k0 = tile * kBlock;
+    if (k0 + kBlock > ptc.n) return;
+    PtcTile& T = tiles[stage];
+    mbar_expect_tx(&full[stage], kTileBytes);
+    tma_load_1d(T.x1, ptc.x1 + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.x2, ptc.x2 + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.x3, ptc.x3 + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.u1, ptc.u1 + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.u2, ptc.u2 + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.u3, ptc.u3 + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.w, ptc.w + k0, kBlock * 8, &full[stage]);
+    tma_load_1d(T.flag, ptc.flag + k0, kBlock * 4, &full[stage]);
+  };
+  if (tid == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (tid == 0 && (int64_t)blockIdx.x < ntiles) issue(blockIdx.x, 0);
+
+  int it = 0;
+  for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+  const int stage = it & 1;
+  PtcTile& T = tiles[stage];
+  const int64_t k = tile * kBlock + tid;
+  if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x, stage ^ 1);
+  if (tile * kBlock + kBlock <= ptc.n) {
+    mbar_wait(&full[stage], (uint32_t)(it >> 1) & 1u);
+  } else {                                          // partial last tile
+    if (k < ptc.n) {
+      T.x1[tid] = ptc.x1[k]; T.x2[tid] = ptc.x2[k]; T.x3[tid] = ptc.x3[k];
+      T.u1[tid] = ptc.u1[k]; T.u2[tid] = ptc.u2[k]; T.u3[tid] = ptc.u3[k];
+      T.w[tid] = ptc.w[k];
+      T.flag[tid] = ptc.flag[k];
+    } else {
+      T.flag[tid] = 2u;
+    }
+    __syncthreads();
+  }
+  const uint32_t flag = T.flag[tid];
+  const bool active = !(flag & 2u);
+
+  // deposit inputs; defaults describe "no contribution"
+  double Q = 0.0, vphi = 0.0, fx = 0.5, fy = 0.5, dx = 1.5, dy = 1.5;
+  uint32_t anchor = 0xFFFFFFFFu;
+
+  if (active) {
+    const double x1 = T.x1[tid], x2 = T.x2[tid];
+    const double sgn = (flag & 1u) ? 1.0 : -1.0;
+
+    // ---- gather (first order, each component from its own staggered lattice): the 24
+    // loads are issued first, exp / sincos / metric run while they are in flight ----
+    const double xa = (x1 - g.xi_in) * g.inv_dxi, ya = x2 * g.inv_dth;
+    const double fin = floor(xa), fjn = floor(ya);
+    const int ia = (int)fin, ja = (int)fjn;
+    const double fih = floor(xa - 0.5), fjh = floor(ya - 0.5);
+    const int ih = (int)fih, jh = (int)fjh;
+    const uint32_t bnn = (uint32_t)g.idx(ia, ja), bhn = (uint32_t)g.idx(ih, ja);
+    const uint32_t bnh = (uint32_t)g.idx(ia, jh), bhh = (uint32_t)g.idx(ih, jh);
+    double G[6][4];
+    {
+      const double* F6[6] = {f.Dr, f.Dth, f.Dph, f.Br, f.Bth, f.Bph};
+      const uint32_t b6[6] = {bhn, bnh, bnn, bnh, bhn, bhh};
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        G[c][0] = __ldg(F6[c] + b6[c]);
+        G[c][1] = __ldg(F6[c] + b6[c] + 1);
+        G[c][2] = __ldg(F6[c] + b6[c] + g.pitch);
+        G[c][3] = __ldg(F6[c] + b6[c] + g.pitch + 1);
+      }
+    }
+
+    // ---- metric at x^n ----
+    const double r0 = exp(x1);
+    double s0, c0;
+    sincos(x2, &s0, &c0);
+    const Pos p0 = make_pos(g, r0, s0, c0);
+
+    double D[3], B[3];
+    {
+      const double wxn = xa - fin, wyn = ya - fjn, wxh = xa - 0.5 - fih, wyh = ya - 0.5 - fjh;
+      const double wx6[6] = {wxh, wxn, wxn, wxn, wxh, wxh};
+      const double wy6[6] = {wyn, wyh, wyn, wyh, wyn, wyh};
+      double V6[6];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) {
+        const double lo = fma(wx6[c], G[c][1] - G[c][0], G[c][0]);
+        const double hi = fma(wx6[c], G[c][3] - G[c][2], G[c][2]);
+        V6[c] = fma(wy6[c], hi - lo, lo);
+      }
+      D[0] = V6[0]; D[1] = V6[1]; D[2] = V6[2]; B[0] = V6[3]; B[1] = V6[4]; B[2] = V6[5];
+    }
+
+    // ---- Boris (full dt) at x^n ----
+    double ur = T.u1[tid], ut = T.u2[tid], up = T.u3[tid];
+    boris(g, p0, sgn, dt, D, B, ur, ut, up);
+
+    // ---- geodesic predictor + K correctors (Eq.14, 15) ----
+    double Xr0, Xt0, Xp0, Ur0, Ut0;
+    geodesic_rhs(g, p0, ur, ut, up, Xr0, Xt0, Xp0, Ur0, Ut0);
+    double dr = Xr0 * dt, dth = Xt0 * dt, dph = Xp0 * dt;      // increments from x^n
+    double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
+    const double hdt = 0.5 * dt;
+    for (int ci = 0; ci < K; ++ci) {
+      double s, c;
+      if (fabs(dth) <= 0.06) sincos_shift(s0, c0, dth, s, c);
+      else sincos(x2 + dth, &s, &c);
+      const Pos p1 = make_pos(g, r0 + dr, s, c);
+      double Xr, Xt, Xp, Ur, Ut;
+      geodesic_rhs(g, p1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
+      dr = hdt * (Xr + Xr0);
+      dth = hdt * (Xt + Xt0);
+      dph = hdt * (Xp + Xp0);
+      vr = fma(hdt, Ur + Ur0, ur);
+      vt = fma(hdt, Ut + Ut0, ut);
+    }
+    const double r = r0 + dr, ph = T.x3[tid] + dph;
+    double th = x2 + dth;
+
+    // ---- new logical position: ln r = x1 + 2 atanh(dr / (2 r0 + dr)) ----
+    double x1n;
+    {
+      const double wq = dr * rcp_nr(r0 + r);
+      if (fabs(wq) <= 0.03) {
+        const double w2 = wq * wq;
+        double pl = fma(w2, 1.0 / 11.0, 1.0 / 9.0);
+        pl = fma(pl, w2, 1.0 / 7.0);
+        pl = fma(pl, w2, 1.0 / 5.0);
+        pl = fma(pl, w2, 1.0 / 3.0);
+        const double at = fma(pl * w2, wq, wq);
+        x1n = fma(2.0, at, x1);
+      } else {
+        x1n = log(r);
+      }
+    }
+    // ---- reflection, removal, new cell ----
+    const double th_dep = th;
+    if (th < 0.0) { th = -th; vt = -vt; }
+    if (th > M_PI) { th = 2.0 * M_PI - th; vt = -vt; }
+    const double xb = (x1n - g.xi_in) * g.inv_dxi, yb = th_dep * g.inv_dth;
+    uint32_t nflag = flag, ncell;
+    const bool finite = isfinite(x1n) && isfinite(th) && isfinite(ph) && isfinite(vr) && isfinite(vt);
+    const bool out = !finite || (x1n < g.xi_in) || (x1n >= g.xi_out);
+    if (out) {
+      nflag |= 2u;
+      ncell = 0xFFFFFFFFu;
+      if (!finite && status) atomicOr(status, GRPIC_STATUS_NONFINITE);
+    } else {
+      // cell = floor of the quotient; the product form decides unless it is within 1e-7 of
+      // a cell edge, where the quotient itself is taken (same decision as a division)
+      double cx = xb, cy = th * g.inv_dth;
+      if (fabs(cx - rint(cx)) < 1e-7) cx = (x1n - g.xi_in) / g.dxi;
+      if (fabs(cy - rint(cy)) < 1e-7) cy = th / g.dth;
+      int ic = (int)floor(cx), jc = (int)floor(cy);
+      ic = min(max(ic, 0), g.nr - 1);
+      jc = min(max(jc, 0), g.nth - 1);
+      ncell = (uint32_t)(jc * g.nr + ic);
+    }
+    ptc.x1[k] = x1n; ptc.x2[k] = th; ptc.x3[k] = ph;
+    ptc.u1[k] = vr; ptc.u2[k] = vt; ptc.u3[k] = up;
+    ptc.cell[k] = ncell;
+    ptc.flag[k] = nflag;
+
+    // ---- deposit set-up: window anchored at (ia-1, ja-1) ----
+    if (finite) {
+      const double q = sgn * T.w[tid];
+      const double vph = q * dph * idt;
+      const double ddx = xb - (double)(ia - 1), ddy = yb - (double)(ja - 1);   // in [0,3) if near
+      const bool near = (ddx >= 0.0) && (ddx < 3.0) && (ddy >= 0.0) && (ddy < 3.0);
+      const bool ingrid = (ia - 1 >= -g.ng) && (ia + 2 <= g.nr + g.ng) && (ja - 1 >= -g.ng) &&
+                          (ja + 2 <= g.nth + g.ng);
+      if (near && ingrid) {
+        Q = q; vphi = vph; fx = xa - fin; fy = ya - fjn; dx = ddx; dy = ddy;
+        anchor = (uint32_t)g.idx(ia - 1, ja - 1);
+      } else {
+        deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
+      }
+    }
+  }
+  deposit_warp(g, J, st, lane, Q, vphi, fx, fy, dx, dy, anchor, idt);
+  __syncthreads();                                  // stage `stage` may be refilled next iteration
+  }
+}
+
+template <int MINB>
+int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_fields& f,
+                        const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
+  static int per_sm = 0;   // resident CTAs per SM of this instantiation
+  if (per_sm == 0) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB>, kBlock, 0) !=
+            cudaSuccess || per_sm < 1)
+      per_sm = 1;
+  }
+  const int64_t ntiles = (ptc.n + kBlock - 1) / kBlock;
+  const int64_t resident = (int64_t)ctx->sm_count * per_sm;
+  const unsigned grid = (unsigned)(ntiles < resident ? ntiles : resident);
+  push_deposit_kernel<MINB><<<grid, kBlock, 0, st>>>(ctx->g, ptc, f, J, dt, ctx->p.geo_iters, status);
+  return grpic_launch_ok();
 }
 
 }  // namespace
@@ -451,11 +588,21 @@ extern "C" int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const gr
   if (!fields->Dr || !fields->Dth || !fields->Dph || !fields->Br || !fields->Bth || !fields->Bph ||
       !flux->Fr || !flux->Fth || !flux->Fph)
     return GRPIC_ERR_ARG;
+  // the particle tiles are fetched with 1-D bulk TMA copies: 16-byte aligned arrays
+  const uintptr_t align = (uintptr_t)ptc->x1 | (uintptr_t)ptc->x2 | (uintptr_t)ptc->x3 |
+                          (uintptr_t)ptc->u1 | (uintptr_t)ptc->u2 | (uintptr_t)ptc->u3 |
+                          (uintptr_t)ptc->w | (uintptr_t)ptc->flag;
+  if (align & 15u) return GRPIC_ERR_ARG;
   if (ptc->n == 0) return GRPIC_OK;
-  const int64_t grid = (ptc->n + kBlock - 1) / kBlock;
-  if (grid > 0x7FFFFFFFLL) return GRPIC_ERR_ARG;
-  push_deposit_kernel<4><<<(unsigned)grid, kBlock, 0, (cudaStream_t)stream>>>(
-      ctx->g, *ptc, *fields, *flux, dt, ctx->p.geo_iters, status);
+  if (ptc->n > 0xFFFFFFF0LL) return GRPIC_ERR_ARG;
+  static int minb = -1;
+  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 4; }
+  cudaStream_t st = (cudaStream_t)stream;
+  int rc;
+  if (minb == 8) rc = launch_push_deposit<8>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (minb == 6) rc = launch_push_deposit<6>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (minb == 5) rc = launch_push_deposit<5>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else rc = launch_push_deposit<4>(ctx, *ptc, *fields, *flux, dt, status, st);
   grpic_count_launches(1);
-  return grpic_launch_ok();
+  return rc;
 }
