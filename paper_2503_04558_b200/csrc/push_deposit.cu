@@ -9,15 +9,14 @@
 // Closed forms: Appendix A with M restored; derivative forms are this
 // file's own.
 //
-// Deposit (Eq.21-23): every particle produces the fluxes of its move on the
-// 4x4 node window anchored one node below its OLD cell (12 F_r faces, 12 F_theta faces, 16
-// F_phi nodes).  Particles are cell-sorted, so the lanes of a warp form a few runs of equal
-// window anchor.  Each warp transposes its 32 x 40 contributions through a private
-// shared-memory tile (slot-major, padded to 33) in two halves of 20 slots; lane L then sums
-// five slots over four consecutive particles, run by run, and issues one red.global.add.f64
-// per (run piece, slot): 10 warp-wide RED instructions with 8-way address sharing instead of
-// 21-40 with 32-way sharing.  Warps with many runs (unsorted or very sparse input) fall back to per-lane
-// reductions of their non-zero values.
+// Deposit (Eq.21-23): every particle adds the fluxes of its move to the
+// 3x3-node window anchored at the lower of its old and new cell (2x3 F_r faces, 3x2 F_theta
+// faces, 3x3 F_phi nodes) with RED.E.ADD.F64; the slots that vanish unless the move crosses a
+// cell face are grouped behind two tests, so a particle issues 8 / 13 / 21 REDs and no
+// per-slot branch.  Measured on B200 (profiles/r01c): the cell sort decays within a few steps
+// (particles move up to half a cell per step), so schemes that reduce runs of equal cell inside
+// a warp before the atomics (v2/v3 of this file) only pay right after a sort, while their
+// per-slot zero tests cost ~200 control instructions per particle afterwards.
 #include <math.h>
 #include <stdlib.h>
 
@@ -26,10 +25,6 @@
 namespace {
 
 constexpr int kBlock = 128;
-constexpr int kSlots = 40;           // 12 F_r + 12 F_theta + 16 F_phi slots of the 4x4 window
-constexpr int kPad = 33;             // particles per slot row (+1 against bank conflicts)
-constexpr unsigned kFull = 0xffffffffu;
-constexpr int kDirectRuns = 12;      // more runs than this in a warp: per-lane reductions
 
 // 1/x: MUFU.RCP64H seed + two Newton steps (~1 ulp); no special-case slow path.
 __device__ __forceinline__ double rcp_nr(double x) {
@@ -149,10 +144,14 @@ __device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double sgn
   ur = fma(k, Dr, pr); ut = fma(k, Dt, pt); up = fma(k, Dp, pp);
 }
 
+// F[...] += v unless v == 0: one DSETP + one predicated RED.E.ADD.F64 (no divergent branch, so
+// no BSSY/BSYNC pair around every one of the 40 window slots).
 __device__ __forceinline__ void red_add(double* p, double v) {
-  if (v != 0.0) atomicAdd(p, v);   // result unused -> RED.E.ADD.F64
+  asm volatile(
+      "{ .reg .pred q; setp.neu.f64 q, %1, 0d0000000000000000; @q red.global.add.f64 [%0], %1; }" ::"l"(p),
+      "d"(v)
+      : "memory");
 }
-
 // sin, cos of th0 + d from (s0, c0) for |d| <= 0.06 (angle addition, Taylor in d).
 __device__ __forceinline__ void sincos_shift(double s0, double c0, double d, double& s, double& c) {
   const double d2 = d * d;
@@ -203,123 +202,70 @@ __device__ __noinline__ void deposit_far(const GridDev* gp, double Q, double idt
                       (1.0 / 6.0) * (S(xb - i) * S(ya - j) + S(xa - i) * S(yb - j))));
 }
 
-// Run reduction of one staged 20 x 32 half-tile (phase ph = slots 20*ph .. 20*ph+19).  Lane L
-// owns the five slots 5*(L&3)..+4 of the phase for the four particles 4*(L>>2)..+3: it sums
-// them in particle order in five independent accumulators and adds the partial sums to
-// F[anchor + off] wherever a run of equal window anchor ends inside its range (and at the end
-// of the range).  `ends` = run ends | 0x88888888.
-__device__ __forceinline__ void reduce_runs(const double* st, int lane, uint32_t ends,
-                                            uint32_t anchor, double* const F[5]) {
-  const int p0 = (lane >> 2) * 4;
-  const double* row = st + (lane & 3) * 5 * kPad + p0;
-  const uint32_t mine = ends >> p0;
-  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-#pragma unroll
-  for (int q = 0; q < 4; ++q) {
-    const uint32_t b = __shfl_sync(kFull, anchor, p0 + q);
-#pragma unroll
-    for (int m = 0; m < 5; ++m) acc[m] += row[m * kPad + q];
-    if ((mine >> q) & 1u) {
-#pragma unroll
-      for (int m = 0; m < 5; ++m) {
-        if (acc[m] != 0.0) atomicAdd(F[m] + b, acc[m]);
-        acc[m] = 0.0;
-      }
-    }
-  }
-}
-
-// global array + in-window offset of deposit slot t (0..11 F_r, 12..23 F_theta, 24..39 F_phi)
-__device__ __forceinline__ double* slot_target(const grpic_current& J, int t, uint32_t pitch) {
-  if (t < 12) return J.Fr + (uint32_t)(t / 3) * pitch + (uint32_t)(t % 3);
-  if (t < 24) return J.Fth + (uint32_t)((t - 12) / 4) * pitch + (uint32_t)((t - 12) % 4);
-  return J.Fph + (uint32_t)((t - 24) / 4) * pitch + (uint32_t)((t - 24) % 4);
-}
-
-// Warp-cooperative charge-conserving deposit of 32 moves (Eq.21-23).  Per lane: charge Q,
-// azimuthal flux Q dphi/dt, old in-cell offsets (fx, fy) in [0,1), new window offsets (dx, dy)
-// in [0,3), window anchor index (0xFFFFFFFF = nothing to deposit; then Q = vphi = 0).
-__device__ __forceinline__ void deposit_warp(const GridDev& g, const grpic_current& J, double* st,
-                                             int lane, double Q, double vphi, double fx, double fy,
-                                             double dx, double dy, uint32_t anchor, double idt) {
-  // shapes on the 4 window nodes: old position (cell-relative fx in [0,1)), new position d in [0,3)
-  const double Sa1 = 1.0 - fx, Sa2 = fx, Ta1 = 1.0 - fy, Ta2 = fy;
-  double Sb[4], Tb[4];
-#pragma unroll
-  for (int m = 0; m < 4; ++m) {
-    Sb[m] = fmax(0.0, 1.0 - fabs(dx - (double)m));
-    Tb[m] = fmax(0.0, 1.0 - fabs(dy - (double)m));
-  }
-  const uint32_t nxt = __shfl_down_sync(kFull, anchor, 1);
-  const uint32_t runs = __ballot_sync(kFull, (lane == 31) || (nxt != anchor));
-  const bool direct = __popc(runs) > kDirectRuns;
+// Charge-conserving deposit of one move (Eq.21-23) on the 3x3-node window anchored at the
+// lower of the old and new cell in each direction: a move of less than one cell touches at
+// most two cells per direction, so 2 F_r faces x 3 rows, 3 columns x 2 F_theta faces and 3x3
+// F_phi nodes hold every non-zero flux.  xa, ya (old) and xb, yb (new) are window-relative
+// logical coordinates in [0,2].  21 unconditional RED.E.ADD.F64 (zeros included): no
+// per-slot zero test, hence no divergent branch around the atomics.
+template <bool GROUPED>
+__device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t anchor, uint32_t pitch,
+                                              double Q, double vphi, double idt, double xa, double ya,
+                                              double xb, double yb, bool cx, bool cy) {
+  // CIC shapes on nodes 0,1,2:  S0 = max(0,1-x), S2 = max(0,x-1), S1 = 1-S0-S2
+  const double Sa0 = fmax(0.0, 1.0 - xa), Sa2 = fmax(0.0, xa - 1.0), Sa1 = (1.0 - Sa0) - Sa2;
+  const double Sb0 = fmax(0.0, 1.0 - xb), Sb2 = fmax(0.0, xb - 1.0), Sb1 = (1.0 - Sb0) - Sb2;
+  const double Ta0 = fmax(0.0, 1.0 - ya), Ta2 = fmax(0.0, ya - 1.0), Ta1 = (1.0 - Ta0) - Ta2;
+  const double Tb0 = fmax(0.0, 1.0 - yb), Tb2 = fmax(0.0, yb - 1.0), Tb1 = (1.0 - Tb0) - Tb2;
   const double hq = -0.5 * Q * idt;
-  // prefix sums of the shape differences (Eq.21): faces 0..2 of the window
-  const double Px0 = Sb[0], Px1 = Px0 + (Sb[1] - Sa1), Px2 = Px1 + (Sb[2] - Sa2);
-  const double Py0 = Tb[0], Py1 = Py0 + (Tb[1] - Ta1), Py2 = Py1 + (Tb[2] - Ta2);
-  const double Ay[4] = {hq * Tb[0], hq * (Tb[1] + Ta1), hq * (Tb[2] + Ta2), hq * Tb[3]};
-  const double Ax[4] = {hq * Sb[0], hq * (Sb[1] + Sa1), hq * (Sb[2] + Sa2), hq * Sb[3]};
-  const double Px[3] = {Px0, Px1, Px2}, Py[3] = {Py0, Py1, Py2};
-  // F_phi (Eq.23): Sb_i U_j + Sa_i V_j
-  double U[4], V[4];
-  {
-    const double c3 = vphi * (1.0 / 3.0), c6 = vphi * (1.0 / 6.0);
-    U[0] = c3 * Tb[0]; U[3] = c3 * Tb[3];
-    U[1] = fma(c3, Tb[1], c6 * Ta1); U[2] = fma(c3, Tb[2], c6 * Ta2);
-    V[0] = c6 * Tb[0]; V[3] = c6 * Tb[3];
-    V[1] = fma(c3, Ta1, c6 * Tb[1]); V[2] = fma(c3, Ta2, c6 * Tb[2]);
-  }
-  const uint32_t pitch = (uint32_t)g.pitch;
-  if (direct) {
-    if (anchor != 0xFFFFFFFFu) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-#pragma unroll
-        for (int m = 0; m < 3; ++m) red_add(J.Fr + anchor + j * pitch + m, Ay[j] * Px[m]);
-#pragma unroll
-      for (int m = 0; m < 3; ++m)
-#pragma unroll
-        for (int i = 0; i < 4; ++i) red_add(J.Fth + anchor + m * pitch + i, Ax[i] * Py[m]);
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        red_add(J.Fph + anchor + j * pitch + 0, Sb[0] * U[j]);
-        red_add(J.Fph + anchor + j * pitch + 1, fma(Sb[1], U[j], Sa1 * V[j]));
-        red_add(J.Fph + anchor + j * pitch + 2, fma(Sb[2], U[j], Sa2 * V[j]));
-        red_add(J.Fph + anchor + j * pitch + 3, Sb[3] * U[j]);
+  // prefix sums of the shape differences over the two faces (Eq.21); the third vanishes
+  const double Px0 = Sb0 - Sa0, Px1 = Sa2 - Sb2;
+  const double Py0 = Tb0 - Ta0, Py1 = Ta2 - Tb2;
+  const double Ay0 = hq * (Tb0 + Ta0), Ay1 = hq * (Tb1 + Ta1), Ay2 = hq * (Tb2 + Ta2);
+  const double Ax0 = hq * (Sb0 + Sa0), Ax1 = hq * (Sb1 + Sa1), Ax2 = hq * (Sb2 + Sa2);
+  // F_phi (Eq.23) = Sb_i U_j + Sa_i V_j
+  const double c3 = vphi * (1.0 / 3.0), c6 = vphi * (1.0 / 6.0);
+  const double U0 = fma(c3, Tb0, c6 * Ta0), U1 = fma(c3, Tb1, c6 * Ta1), U2 = fma(c3, Tb2, c6 * Ta2);
+  const double V0 = fma(c3, Ta0, c6 * Tb0), V1 = fma(c3, Ta1, c6 * Tb1), V2 = fma(c3, Ta2, c6 * Tb2);
+  double* fr = J.Fr + anchor;
+  double* ft = J.Fth + anchor;
+  double* fp = J.Fph + anchor;
+  const uint32_t p2 = 2u * pitch;
+  if (!GROUPED) {
+    atomicAdd(fr, Ay0 * Px0);          atomicAdd(fr + 1, Ay0 * Px1);
+    atomicAdd(fr + pitch, Ay1 * Px0);  atomicAdd(fr + pitch + 1, Ay1 * Px1);
+    atomicAdd(fr + p2, Ay2 * Px0);     atomicAdd(fr + p2 + 1, Ay2 * Px1);
+    atomicAdd(ft, Ax0 * Py0);          atomicAdd(ft + 1, Ax1 * Py0);          atomicAdd(ft + 2, Ax2 * Py0);
+    atomicAdd(ft + pitch, Ax0 * Py1);  atomicAdd(ft + pitch + 1, Ax1 * Py1);  atomicAdd(ft + pitch + 2, Ax2 * Py1);
+    atomicAdd(fp, fma(Sb0, U0, Sa0 * V0));          atomicAdd(fp + 1, fma(Sb1, U0, Sa1 * V0));
+    atomicAdd(fp + 2, fma(Sb2, U0, Sa2 * V0));
+    atomicAdd(fp + pitch, fma(Sb0, U1, Sa0 * V1));  atomicAdd(fp + pitch + 1, fma(Sb1, U1, Sa1 * V1));
+    atomicAdd(fp + pitch + 2, fma(Sb2, U1, Sa2 * V1));
+    atomicAdd(fp + p2, fma(Sb0, U2, Sa0 * V2));     atomicAdd(fp + p2 + 1, fma(Sb1, U2, Sa1 * V2));
+    atomicAdd(fp + p2 + 2, fma(Sb2, U2, Sa2 * V2));
+  } else {
+    // slots that vanish unless the move crosses a cell face in xi (cx) / theta (cy) are
+    // grouped behind those two tests: 8 always, +5 if cx, +5 if cy, +3 if both
+    atomicAdd(fr, Ay0 * Px0);          atomicAdd(fr + pitch, Ay1 * Px0);
+    atomicAdd(ft, Ax0 * Py0);          atomicAdd(ft + 1, Ax1 * Py0);
+    atomicAdd(fp, fma(Sb0, U0, Sa0 * V0));          atomicAdd(fp + 1, fma(Sb1, U0, Sa1 * V0));
+    atomicAdd(fp + pitch, fma(Sb0, U1, Sa0 * V1));  atomicAdd(fp + pitch + 1, fma(Sb1, U1, Sa1 * V1));
+    if (cx) {
+      atomicAdd(fr + 1, Ay0 * Px1);    atomicAdd(fr + pitch + 1, Ay1 * Px1);
+      atomicAdd(ft + 2, Ax2 * Py0);
+      atomicAdd(fp + 2, fma(Sb2, U0, Sa2 * V0));    atomicAdd(fp + pitch + 2, fma(Sb2, U1, Sa2 * V1));
+    }
+    if (cy) {
+      atomicAdd(fr + p2, Ay2 * Px0);
+      atomicAdd(ft + pitch, Ax0 * Py1);  atomicAdd(ft + pitch + 1, Ax1 * Py1);
+      atomicAdd(fp + p2, fma(Sb0, U2, Sa0 * V2));   atomicAdd(fp + p2 + 1, fma(Sb1, U2, Sa1 * V2));
+      if (cx) {
+        atomicAdd(fr + p2 + 1, Ay2 * Px1);
+        atomicAdd(ft + pitch + 2, Ax2 * Py1);
+        atomicAdd(fp + p2 + 2, fma(Sb2, U2, Sa2 * V2));
       }
     }
-    return;
   }
-  // slots 0..11 = F_r (row j, face m), 12..23 = F_theta (face m, column i), 24..39 = F_phi;
-  // staged and reduced in two halves of 20 slots
-#pragma unroll
-  for (int j = 0; j < 4; ++j)
-#pragma unroll
-    for (int m = 0; m < 3; ++m) st[(j * 3 + m) * kPad + lane] = Ay[j] * Px[m];
-#pragma unroll
-  for (int m = 0; m < 2; ++m)
-#pragma unroll
-    for (int i = 0; i < 4; ++i) st[(12 + m * 4 + i) * kPad + lane] = Ax[i] * Py[m];
-  __syncwarp();
-  const uint32_t ends = runs | 0x88888888u;
-  double* F[5];
-#pragma unroll
-  for (int m = 0; m < 5; ++m) F[m] = slot_target(J, (lane & 3) * 5 + m, pitch);
-  reduce_runs(st, lane, ends, anchor, F);
-  __syncwarp();
-#pragma unroll
-  for (int i = 0; i < 4; ++i) st[i * kPad + lane] = Ax[i] * Py[2];
-#pragma unroll
-  for (int j = 0; j < 4; ++j) {
-    st[(4 + j * 4 + 0) * kPad + lane] = Sb[0] * U[j];
-    st[(4 + j * 4 + 1) * kPad + lane] = fma(Sb[1], U[j], Sa1 * V[j]);
-    st[(4 + j * 4 + 2) * kPad + lane] = fma(Sb[2], U[j], Sa2 * V[j]);
-    st[(4 + j * 4 + 3) * kPad + lane] = Sb[3] * U[j];
-  }
-  __syncwarp();
-#pragma unroll
-  for (int m = 0; m < 5; ++m) F[m] = slot_target(J, 20 + (lane & 3) * 5 + m, pitch);
-  reduce_runs(st, lane, ends, anchor, F);
 }
 
 // ---- TMA (cp.async.bulk) + mbarrier plumbing for the double-buffered particle tiles ----
@@ -351,60 +297,66 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
       : "memory");
 }
 
-// One tile of particle input staged in shared memory (structure of arrays, 128 particles).
+// One warp tile of particle input staged in shared memory (structure of arrays, 32 particles).
+constexpr int kWarps = kBlock / 32;
 struct __align__(128) PtcTile {
-  double x1[kBlock], x2[kBlock], x3[kBlock], u1[kBlock], u2[kBlock], u3[kBlock], w[kBlock];
-  uint32_t flag[kBlock];
+  double x1[32], x2[32], x3[32], u1[32], u2[32], u3[32], w[32];
+  uint32_t flag[32];
 };
-constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
+constexpr uint32_t kTileBytes = 7u * 32u * 8u + 32u * 4u;
 
-// Persistent kernel: each CTA walks the 128-particle tiles blockIdx.x, +gridDim.x, ...; the
-// particle state of the NEXT tile is fetched by eight 1-D bulk TMA copies into the other
-// shared-memory stage while the current tile is pushed, so no warp waits on a DRAM round trip
-// for its particle.  The last, partial tile (n % 128 != 0) is staged with plain loads.
-template <int MINB>
+// Persistent kernel, warp-autonomous: every warp walks its own 32-particle tiles
+// (global warp id, + total warps, ...).  The particle state of a warp's NEXT tile is fetched by
+// eight 1-D bulk TMA copies into the warp's other shared-memory stage while the current tile
+// is pushed.  No block-wide barrier exists: a warp that takes a slow path (far deposit,
+// large-angle sincos) delays nobody.  The last, partial tile (n % 32 != 0) is staged
+// with plain loads.
+template <int MINB, bool GROUPED, int KT>
 __global__ void __launch_bounds__(kBlock, MINB)
 push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
                     const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
                     double dt, int K, uint32_t* status) {
-  __shared__ PtcTile tiles[2];
-  __shared__ __align__(8) uint64_t full[2];
-  __shared__ double stage_all[kBlock / 32][(kSlots / 2) * kPad];
-  const int tid = threadIdx.x, lane = tid & 31;
-  double* st = stage_all[tid >> 5];
-  const int64_t ntiles = (ptc.n + kBlock - 1) / kBlock;
+  __shared__ PtcTile tiles[kWarps][2];
+  __shared__ __align__(8) uint64_t full[kWarps][2];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int tid = lane;                              // index inside the warp tile
+  const int64_t ntiles = (ptc.n + 31) / 32;
+  const int64_t tstride = (int64_t)gridDim.x * kWarps;
   const double idt = 1.0 / dt;
 
-  auto issue = [&](int64_t tile, int stage) {       // thread 0 only; full tiles only
-    const int64_t k0 = tile * kBlock;
-    if (k0 + kBlock > ptc.n) return;
-    PtcTile& T = tiles[stage];
-    mbar_expect_tx(&full[stage], kTileBytes);
-    tma_load_1d(T.x1, ptc.x1 + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.x2, ptc.x2 + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.x3, ptc.x3 + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.u1, ptc.u1 + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.u2, ptc.u2 + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.u3, ptc.u3 + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.w, ptc.w + k0, kBlock * 8, &full[stage]);
-    tma_load_1d(T.flag, ptc.flag + k0, kBlock * 4, &full[stage]);
+  auto issue = [&](int64_t tile, int stage) {       // lane 0 only; full tiles only
+    const int64_t k0 = tile * 32;
+    if (k0 + 32 > ptc.n) return;
+    PtcTile& T = tiles[warp][stage];
+    uint64_t* bar = &full[warp][stage];
+    mbar_expect_tx(bar, kTileBytes);
+    tma_load_1d(T.x1, ptc.x1 + k0, 256, bar);
+    tma_load_1d(T.x2, ptc.x2 + k0, 256, bar);
+    tma_load_1d(T.x3, ptc.x3 + k0, 256, bar);
+    tma_load_1d(T.u1, ptc.u1 + k0, 256, bar);
+    tma_load_1d(T.u2, ptc.u2 + k0, 256, bar);
+    tma_load_1d(T.u3, ptc.u3 + k0, 256, bar);
+    tma_load_1d(T.w, ptc.w + k0, 256, bar);
+    tma_load_1d(T.flag, ptc.flag + k0, 128, bar);
   };
-  if (tid == 0) {
-    mbar_init(&full[0], 1);
-    mbar_init(&full[1], 1);
+  const int64_t tile0 = (int64_t)blockIdx.x * kWarps + warp;
+  if (lane == 0) {
+    mbar_init(&full[warp][0], 1);
+    mbar_init(&full[warp][1], 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    if (tile0 < ntiles) issue(tile0, 0);
   }
-  __syncthreads();
-  if (tid == 0 && (int64_t)blockIdx.x < ntiles) issue(blockIdx.x, 0);
+  __syncwarp();
 
   int it = 0;
-  for (int64_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+  for (int64_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
   const int stage = it & 1;
-  PtcTile& T = tiles[stage];
-  const int64_t k = tile * kBlock + tid;
-  if (tid == 0 && tile + gridDim.x < ntiles) issue(tile + gridDim.x, stage ^ 1);
-  if (tile * kBlock + kBlock <= ptc.n) {
-    mbar_wait(&full[stage], (uint32_t)(it >> 1) & 1u);
+  PtcTile& T = tiles[warp][stage];
+  const int64_t k = tile * 32 + lane;
+  const int64_t tnext = tile + tstride;
+  if (lane == 0 && tnext < ntiles) issue(tnext, stage ^ 1);
+  if (tile * 32 + 32 <= ptc.n) {
+    mbar_wait(&full[warp][stage], (uint32_t)(it >> 1) & 1u);
   } else {                                          // partial last tile
     if (k < ptc.n) {
       T.x1[tid] = ptc.x1[k]; T.x2[tid] = ptc.x2[k]; T.x3[tid] = ptc.x3[k];
@@ -414,14 +366,10 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     } else {
       T.flag[tid] = 2u;
     }
-    __syncthreads();
+    __syncwarp();
   }
   const uint32_t flag = T.flag[tid];
   const bool active = !(flag & 2u);
-
-  // deposit inputs; defaults describe "no contribution"
-  double Q = 0.0, vphi = 0.0, fx = 0.5, fy = 0.5, dx = 1.5, dy = 1.5;
-  uint32_t anchor = 0xFFFFFFFFu;
 
   if (active) {
     const double x1 = T.x1[tid], x2 = T.x2[tid];
@@ -480,7 +428,9 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     double dr = Xr0 * dt, dth = Xt0 * dt, dph = Xp0 * dt;      // increments from x^n
     double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
     const double hdt = 0.5 * dt;
-    for (int ci = 0; ci < K; ++ci) {
+    const int KK = KT > 0 ? KT : K;                 // KT: compile-time corrector count (unrolled)
+#pragma unroll
+    for (int ci = 0; ci < KK; ++ci) {
       double s, c;
       if (fabs(dth) <= 0.06) sincos_shift(s0, c0, dth, s, c);
       else sincos(x2 + dth, &s, &c);
@@ -540,40 +490,40 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     ptc.cell[k] = ncell;
     ptc.flag[k] = nflag;
 
-    // ---- deposit set-up: window anchored at (ia-1, ja-1) ----
+    // ---- deposit: 3x3 window anchored at the lower of the old / new cell ----
     if (finite) {
       const double q = sgn * T.w[tid];
       const double vph = q * dph * idt;
-      const double ddx = xb - (double)(ia - 1), ddy = yb - (double)(ja - 1);   // in [0,3) if near
-      const bool near = (ddx >= 0.0) && (ddx < 3.0) && (ddy >= 0.0) && (ddy < 3.0);
-      const bool ingrid = (ia - 1 >= -g.ng) && (ia + 2 <= g.nr + g.ng) && (ja - 1 >= -g.ng) &&
-                          (ja + 2 <= g.nth + g.ng);
-      if (near && ingrid) {
-        Q = q; vphi = vph; fx = xa - fin; fy = ya - fjn; dx = ddx; dy = ddy;
-        anchor = (uint32_t)g.idx(ia - 1, ja - 1);
+      const int ib = (int)floor(xb), jb = (int)floor(yb);
+      const int di = ib - ia, dj = jb - ja;
+      if (di >= -1 && di <= 1 && dj >= -1 && dj <= 1) {
+        const int iw = min(ia, ib), jw = min(ja, jb);
+        const double ox = (double)iw, oy = (double)jw;
+        deposit_local<GROUPED>(J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - ox,
+                               ya - oy, xb - ox, yb - oy, di != 0, dj != 0);
       } else {
         deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
       }
     }
   }
-  deposit_warp(g, J, st, lane, Q, vphi, fx, fy, dx, dy, anchor, idt);
-  __syncthreads();                                  // stage `stage` may be refilled next iteration
+  __syncwarp();                                     // stage `stage` may be refilled next iteration
   }
 }
 
-template <int MINB>
+template <int MINB, bool GROUPED, int KT>
 int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_fields& f,
                         const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
   static int per_sm = 0;   // resident CTAs per SM of this instantiation
   if (per_sm == 0) {
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB>, kBlock, 0) !=
-            cudaSuccess || per_sm < 1)
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, GROUPED, KT>,
+                                                      kBlock, 0) != cudaSuccess || per_sm < 1)
       per_sm = 1;
   }
-  const int64_t ntiles = (ptc.n + kBlock - 1) / kBlock;
+  const int64_t nblocks = (ptc.n + kBlock - 1) / kBlock;
   const int64_t resident = (int64_t)ctx->sm_count * per_sm;
-  const unsigned grid = (unsigned)(ntiles < resident ? ntiles : resident);
-  push_deposit_kernel<MINB><<<grid, kBlock, 0, st>>>(ctx->g, ptc, f, J, dt, ctx->p.geo_iters, status);
+  const unsigned grid = (unsigned)(nblocks < resident ? nblocks : resident);
+  push_deposit_kernel<MINB, GROUPED, KT><<<grid, kBlock, 0, st>>>(ctx->g, ptc, f, J, dt,
+                                                                  ctx->p.geo_iters, status);
   return grpic_launch_ok();
 }
 
@@ -595,14 +545,19 @@ extern "C" int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const gr
   if (align & 15u) return GRPIC_ERR_ARG;
   if (ptc->n == 0) return GRPIC_OK;
   if (ptc->n > 0xFFFFFFF0LL) return GRPIC_ERR_ARG;
-  static int minb = -1;
-  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 4; }
+  // tuning knobs (read once): resident CTAs per SM and the grouping of the deposit REDs
+  static int minb = -1, grouped = -1;
+  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 5; }
+  if (grouped < 0) { const char* e = getenv("GRPIC_PD_GROUPED"); grouped = e ? atoi(e) : 1; }
   cudaStream_t st = (cudaStream_t)stream;
   int rc;
-  if (minb == 8) rc = launch_push_deposit<8>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (minb == 6) rc = launch_push_deposit<6>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (minb == 5) rc = launch_push_deposit<5>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else rc = launch_push_deposit<4>(ctx, *ptc, *fields, *flux, dt, status, st);
+  if (ctx->p.geo_iters != 3) rc = launch_push_deposit<4, true, 0>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (minb == 6 && grouped) rc = launch_push_deposit<6, true, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (minb == 6) rc = launch_push_deposit<6, false, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (minb == 5 && grouped) rc = launch_push_deposit<5, true, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (minb == 5) rc = launch_push_deposit<5, false, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else if (grouped) rc = launch_push_deposit<4, true, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
+  else rc = launch_push_deposit<4, false, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
   grpic_count_launches(1);
   return rc;
 }
