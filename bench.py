@@ -63,6 +63,8 @@ def parse():
     ap.add_argument("--grid", type=int, default=0, help="override nr = nth")
     ap.add_argument("--sort-every", type=int, default=-1)
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--separate-compact", action="store_true",
+                    help="run compaction as its own pass instead of fused into the push")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -169,6 +171,7 @@ def run_ours(args):
     sort_every = args.sort_every if args.sort_every >= 0 else (meta.get("sort_every") or 20)
     compact = bool(meta.get("compact_every", 0))
     filt = int(meta.get("filter_passes", 0))
+    fused = compact and not args.separate_compact
 
     ctx = grpic.Context(p, n)
     fields = [ctx.to_device(f) for f in cfg["fields"]]
@@ -195,12 +198,18 @@ def run_ours(args):
             cur, alt = alt, cur
         for f in flux:
             f.zero_()
-        mark(s, "push_deposit", 0); ctx.push_deposit(cur, fields, flux, dt); mark(s, "push_deposit", 1)
+        mark(s, "push_deposit", 0)
+        if fused:       # removal fused into the push: survivors of `cur` are pushed into `alt`
+            ctx.push_deposit_compact(cur, alt, fields, flux, dt, n_alive[s:s + 1])
+            cur, alt = alt, cur
+        else:
+            ctx.push_deposit(cur, fields, flux, dt)
+        mark(s, "push_deposit", 1)
         if world > 1:
             sharding.allreduce_flux(flux)
         mark(s, "finalize", 0); ctx.finalize_current(flux, filt); mark(s, "finalize", 1)
         mark(s, "field_step", 0); ctx.field_step(fields, flux, dt, bg); mark(s, "field_step", 1)
-        if compact:
+        if compact and not fused:
             mark(s, "compact", 0); ctx.compact(cur, alt, n_alive[s:s + 1]); mark(s, "compact", 1)
             cur, alt = alt, cur
         return cur, alt
@@ -240,7 +249,7 @@ def run_ours(args):
     # particles actually pushed per timed step (alive at the start of the step)
     if compact:
         al = n_alive.cpu().numpy()
-        pushed = [n if s == 0 else int(al[s - 1]) for s in range(W, W + K)]
+        pushed = [int(al[s]) if fused else (n if s == 0 else int(al[s - 1])) for s in range(W, W + K)]
     else:
         pushed = [n] * K
     units = float(sum(pushed))
@@ -335,7 +344,10 @@ def run_ours(args):
             "config": {"workload": "BASELINE.json configs[%d]: %dx%d (log r, theta) grid, a=%.2f, "
                                    "%d particles per GPU" % (args.config - 1, p["nr"], p["nth"], p["a"], n),
                        "particles_per_gpu": n, "grid": [p["nr"], p["nth"]], "dt": dt,
-                       "sort_every": sort_every, "compact_every_step": compact, "filter_passes": filt,
+                       "sort_every": sort_every, "compact_every_step": compact,
+                       "compaction": ("fused into the push (grpic_push_deposit_compact)" if fused else
+                                      "separate pass (grpic_compact)") if compact else "none",
+                       "filter_passes": filt,
                        "field_step": True, "field_iters": p["field_iters"], "geo_iters": p["geo_iters"],
                        "macro_weight": BENCH_WEIGHT,
                        "parallelism": "particle-sharded replicas (grid replicated), all-reduce of J"
@@ -375,13 +387,12 @@ def run_e2e(args, ctx, grpic, state, fields0, flux, dt, filt, bg, world, dist):
             cur.t[k].copy_(host[k], non_blocking=True)
         for f in flux:
             f.zero_()
-        ctx.push_deposit(cur, fields, flux, dt)
+        ctx.push_deposit_compact(cur, alt, fields, flux, dt, n_alive)
         if world > 1:
             for f in flux:
                 dist.all_reduce(f)
         ctx.finalize_current(flux, filt)
         ctx.field_step(fields, flux, dt, bg)
-        ctx.compact(cur, alt, n_alive)
         for k in back:
             host[k].copy_(alt.t[k], non_blocking=True)
         for a, b in zip(hJ, flux):
@@ -406,7 +417,7 @@ def run_e2e(args, ctx, grpic, state, fields0, flux, dt, filt, bg, world, dist):
         ms = float(t.item())
     return {"value": float(n) * KE * world / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
             "d2h_bytes_per_step": int(d2h), "steps": KE, "ms_per_step": ms / KE,
-            "path": "pinned host SoA -> H2D -> push+deposit, finalize, field step, compact -> D2H "
+            "path": "pinned host SoA -> H2D -> push+deposit+compaction, finalize, field step -> D2H "
                     "of particle state and J"}
 
 

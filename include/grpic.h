@@ -110,6 +110,18 @@ int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes);
 int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                        grpic_current* flux, double dt, uint32_t* status, void* stream);
 
+/* Removal fused into the push (SURVEY 8(a) rows a1-a5 + a9): exactly
+ * grpic_compact(in -> out) followed by grpic_push_deposit(out), in one pass over the particles.
+ * `out` (must not alias `in`; in is not modified) receives, in their original order, the
+ * particles of `in` that are not flagged removed, each advanced one step (a particle that leaves
+ * during THIS step is stored with its removed flag set and is squeezed out by the next call);
+ * the DEVICE word *n_alive = number of particles pushed (= survivors of `in`); entries
+ * [*n_alive, n) of out are marked removed, so the caller may keep using n as the upper bound
+ * without reading n_alive back.  out->n = in->n.  Needs workspace (one word per 32 particles). */
+int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out,
+                               const grpic_fields* fields, grpic_current* flux, double dt,
+                               int64_t* n_alive, uint32_t* status, void* stream);
+
 /* Fluxes -> current densities, in place: fold the theta ghost rows onto their mirror rows
  * (particles never cross the axis, :136), `filter_passes` passes of the (1,2,1)x(1,2,1)/16
  * binomial filter on the fluxes (BASELINE.json config 5), then J^r = F_r/A^D_r,

@@ -58,3 +58,5 @@ __device__ __forceinline__ double ks_sqrtg(double a2, double M, double r, double
 
 // launch bookkeeping for bench.py's gpu_launches (api.cu)
 void grpic_count_launches(int n);
+// in-place exclusive scan of data[0..n) (sort.cu); scratch >= n/2048 + n/2048^2 + 8 words
+int grpic_exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st);

@@ -206,9 +206,8 @@ __device__ __noinline__ void deposit_far(const GridDev* gp, double Q, double idt
 // lower of the old and new cell in each direction: a move of less than one cell touches at
 // most two cells per direction, so 2 F_r faces x 3 rows, 3 columns x 2 F_theta faces and 3x3
 // F_phi nodes hold every non-zero flux.  xa, ya (old) and xb, yb (new) are window-relative
-// logical coordinates in [0,2].  21 unconditional RED.E.ADD.F64 (zeros included): no
-// per-slot zero test, hence no divergent branch around the atomics.
-template <bool GROUPED>
+// logical coordinates in [0,2].  No per-slot zero test (each costs a divergent branch around
+// the atomic); issuing all 21 REDs unconditionally is LSU-bound (12.5 ms vs 7.1 ms at 1e8).
 __device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t anchor, uint32_t pitch,
                                               double Q, double vphi, double idt, double xa, double ya,
                                               double xb, double yb, bool cx, bool cy) {
@@ -231,19 +230,7 @@ __device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t a
   double* ft = J.Fth + anchor;
   double* fp = J.Fph + anchor;
   const uint32_t p2 = 2u * pitch;
-  if (!GROUPED) {
-    atomicAdd(fr, Ay0 * Px0);          atomicAdd(fr + 1, Ay0 * Px1);
-    atomicAdd(fr + pitch, Ay1 * Px0);  atomicAdd(fr + pitch + 1, Ay1 * Px1);
-    atomicAdd(fr + p2, Ay2 * Px0);     atomicAdd(fr + p2 + 1, Ay2 * Px1);
-    atomicAdd(ft, Ax0 * Py0);          atomicAdd(ft + 1, Ax1 * Py0);          atomicAdd(ft + 2, Ax2 * Py0);
-    atomicAdd(ft + pitch, Ax0 * Py1);  atomicAdd(ft + pitch + 1, Ax1 * Py1);  atomicAdd(ft + pitch + 2, Ax2 * Py1);
-    atomicAdd(fp, fma(Sb0, U0, Sa0 * V0));          atomicAdd(fp + 1, fma(Sb1, U0, Sa1 * V0));
-    atomicAdd(fp + 2, fma(Sb2, U0, Sa2 * V0));
-    atomicAdd(fp + pitch, fma(Sb0, U1, Sa0 * V1));  atomicAdd(fp + pitch + 1, fma(Sb1, U1, Sa1 * V1));
-    atomicAdd(fp + pitch + 2, fma(Sb2, U1, Sa2 * V1));
-    atomicAdd(fp + p2, fma(Sb0, U2, Sa0 * V2));     atomicAdd(fp + p2 + 1, fma(Sb1, U2, Sa1 * V2));
-    atomicAdd(fp + p2 + 2, fma(Sb2, U2, Sa2 * V2));
-  } else {
+  {
     // slots that vanish unless the move crosses a cell face in xi (cx) / theta (cy) are
     // grouped behind those two tests: 8 always, +5 if cx, +5 if cy, +3 if both
     atomicAdd(fr, Ay0 * Px0);          atomicAdd(fr + pitch, Ay1 * Px0);
@@ -311,11 +298,17 @@ constexpr uint32_t kTileBytes = 7u * 32u * 8u + 32u * 4u;
 // is pushed.  No block-wide barrier exists: a warp that takes a slow path (far deposit,
 // large-angle sincos) delays nobody.  The last, partial tile (n % 32 != 0) is staged
 // with plain loads.
-template <int MINB, bool GROUPED, int KT>
+//
+// COMPACT: the results are stored to `dst` at offsets[tile] + rank among the tile's live lanes
+// (offsets = exclusive scan of the per-tile live counts of `ptc`), i.e. particles already
+// flagged removed are squeezed out on the way, order preserved; the weight travels along.
+// Otherwise dst == ptc and the update is in place.
+template <int MINB, bool COMPACT, int KT>
 __global__ void __launch_bounds__(kBlock, MINB)
 push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
-                    const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
-                    double dt, int K, uint32_t* status) {
+                    const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
+                    int64_t* n_alive, const __grid_constant__ grpic_fields f,
+                    const __grid_constant__ grpic_current J, double dt, int K, uint32_t* status) {
   __shared__ PtcTile tiles[kWarps][2];
   __shared__ __align__(8) uint64_t full[kWarps][2];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -370,6 +363,12 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   }
   const uint32_t flag = T.flag[tid];
   const bool active = !(flag & 2u);
+  uint32_t live = 0, obase = 0;
+  if (COMPACT) {
+    live = __ballot_sync(0xffffffffu, active);
+    obase = offsets[tile];
+    if (tile == ntiles - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
+  }
 
   if (active) {
     const double x1 = T.x1[tid], x2 = T.x2[tid];
@@ -485,10 +484,13 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
     }
-    ptc.x1[k] = x1n; ptc.x2[k] = th; ptc.x3[k] = ph;
-    ptc.u1[k] = vr; ptc.u2[k] = vt; ptc.u3[k] = up;
-    ptc.cell[k] = ncell;
-    ptc.flag[k] = nflag;
+    int64_t kd = k;
+    if (COMPACT) kd = (int64_t)obase + __popc(live & ((1u << lane) - 1u));
+    dst.x1[kd] = x1n; dst.x2[kd] = th; dst.x3[kd] = ph;
+    dst.u1[kd] = vr; dst.u2[kd] = vt; dst.u3[kd] = up;
+    if (COMPACT) dst.w[kd] = T.w[tid];
+    dst.cell[kd] = ncell;
+    dst.flag[kd] = nflag;
 
     // ---- deposit: 3x3 window anchored at the lower of the old / new cell ----
     if (finite) {
@@ -499,7 +501,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       if (di >= -1 && di <= 1 && dj >= -1 && dj <= 1) {
         const int iw = min(ia, ib), jw = min(ja, jb);
         const double ox = (double)iw, oy = (double)jw;
-        deposit_local<GROUPED>(J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - ox,
+        deposit_local(J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - ox,
                                ya - oy, xb - ox, yb - oy, di != 0, dj != 0);
       } else {
         deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
@@ -510,54 +512,104 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   }
 }
 
-template <int MINB, bool GROUPED, int KT>
-int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_fields& f,
+template <int MINB, bool COMPACT, int KT>
+int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
+                        const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
                         const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
   static int per_sm = 0;   // resident CTAs per SM of this instantiation
   if (per_sm == 0) {
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, GROUPED, KT>,
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, COMPACT, KT>,
                                                       kBlock, 0) != cudaSuccess || per_sm < 1)
       per_sm = 1;
   }
   const int64_t nblocks = (ptc.n + kBlock - 1) / kBlock;
   const int64_t resident = (int64_t)ctx->sm_count * per_sm;
   const unsigned grid = (unsigned)(nblocks < resident ? nblocks : resident);
-  push_deposit_kernel<MINB, GROUPED, KT><<<grid, kBlock, 0, st>>>(ctx->g, ptc, f, J, dt,
-                                                                  ctx->p.geo_iters, status);
+  push_deposit_kernel<MINB, COMPACT, KT><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, n_alive, f, J,
+                                                                  dt, ctx->p.geo_iters, status);
   return grpic_launch_ok();
+}
+
+template <bool COMPACT>
+int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
+                          const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
+                          const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
+  static int minb = -1;   // tuning knob (read once): resident CTAs per SM
+  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 5; }
+  if (ctx->p.geo_iters != 3)
+    return launch_push_deposit<4, COMPACT, 0>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+  if (minb == 4)
+    return launch_push_deposit<4, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+  return launch_push_deposit<5, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+}
+
+// live particles per 32-particle tile (one warp per tile, ballot)
+__global__ void __launch_bounds__(256) tile_live_kernel(const uint32_t* flag, int64_t n, uint32_t* counts) {
+  const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  const bool live = (k < n) && !(flag[k] & 2u);
+  const uint32_t b = __ballot_sync(0xffffffffu, live);
+  if ((threadIdx.x & 31) == 0 && k < n) counts[k >> 5] = __popc(b);
+}
+// out[k] for k in [*n_alive, n): flag = removed
+__global__ void mark_tail_range_kernel(grpic_particles out, int64_t n, const int64_t* n_alive) {
+  for (int64_t k = *n_alive + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n;
+       k += (int64_t)gridDim.x * blockDim.x) {
+    out.flag[k] = 2u;
+    out.cell[k] = 0xFFFFFFFFu;
+  }
+}
+
+bool ptc_args_ok(const grpic_particles* p) {
+  return p && p->n >= 0 && p->x1 && p->x2 && p->x3 && p->u1 && p->u2 && p->u3 && p->w && p->cell && p->flag;
+}
+bool tma_aligned(const grpic_particles* p) {
+  const uintptr_t a = (uintptr_t)p->x1 | (uintptr_t)p->x2 | (uintptr_t)p->x3 | (uintptr_t)p->u1 |
+                      (uintptr_t)p->u2 | (uintptr_t)p->u3 | (uintptr_t)p->w | (uintptr_t)p->flag;
+  return (a & 15u) == 0;
+}
+bool grid_args_ok(const grpic_fields* f, const grpic_current* J) {
+  return f && J && f->Dr && f->Dth && f->Dph && f->Br && f->Bth && f->Bph && J->Fr && J->Fth && J->Fph;
 }
 
 }  // namespace
 
 extern "C" int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                                   grpic_current* flux, double dt, uint32_t* status, void* stream) {
-  if (!ctx || !ptc || !fields || !flux || !(dt > 0.0) || ptc->n < 0) return GRPIC_ERR_ARG;
-  if (!ptc->x1 || !ptc->x2 || !ptc->x3 || !ptc->u1 || !ptc->u2 || !ptc->u3 || !ptc->w ||
-      !ptc->cell || !ptc->flag)
-    return GRPIC_ERR_ARG;
-  if (!fields->Dr || !fields->Dth || !fields->Dph || !fields->Br || !fields->Bth || !fields->Bph ||
-      !flux->Fr || !flux->Fth || !flux->Fph)
-    return GRPIC_ERR_ARG;
+  if (!ctx || !ptc_args_ok(ptc) || !grid_args_ok(fields, flux) || !(dt > 0.0)) return GRPIC_ERR_ARG;
   // the particle tiles are fetched with 1-D bulk TMA copies: 16-byte aligned arrays
-  const uintptr_t align = (uintptr_t)ptc->x1 | (uintptr_t)ptc->x2 | (uintptr_t)ptc->x3 |
-                          (uintptr_t)ptc->u1 | (uintptr_t)ptc->u2 | (uintptr_t)ptc->u3 |
-                          (uintptr_t)ptc->w | (uintptr_t)ptc->flag;
-  if (align & 15u) return GRPIC_ERR_ARG;
+  if (!tma_aligned(ptc)) return GRPIC_ERR_ARG;
   if (ptc->n == 0) return GRPIC_OK;
   if (ptc->n > 0xFFFFFFF0LL) return GRPIC_ERR_ARG;
-  // tuning knobs (read once): resident CTAs per SM and the grouping of the deposit REDs
-  static int minb = -1, grouped = -1;
-  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 5; }
-  if (grouped < 0) { const char* e = getenv("GRPIC_PD_GROUPED"); grouped = e ? atoi(e) : 1; }
-  cudaStream_t st = (cudaStream_t)stream;
-  int rc;
-  if (ctx->p.geo_iters != 3) rc = launch_push_deposit<4, true, 0>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (minb == 6 && grouped) rc = launch_push_deposit<6, true, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (minb == 6) rc = launch_push_deposit<6, false, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (minb == 5 && grouped) rc = launch_push_deposit<5, true, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (minb == 5) rc = launch_push_deposit<5, false, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else if (grouped) rc = launch_push_deposit<4, true, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
-  else rc = launch_push_deposit<4, false, 3>(ctx, *ptc, *fields, *flux, dt, status, st);
+  const int rc = dispatch_push_deposit<false>(ctx, *ptc, *ptc, nullptr, nullptr, *fields, *flux, dt, status,
+                                              (cudaStream_t)stream);
   grpic_count_launches(1);
   return rc;
+}
+
+extern "C" int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out,
+                                          const grpic_fields* fields, grpic_current* flux, double dt,
+                                          int64_t* n_alive, uint32_t* status, void* stream) {
+  if (!ctx || !in || in->n < 0 || !out || !n_alive || !grid_args_ok(fields, flux) || !(dt > 0.0))
+    return GRPIC_ERR_ARG;
+  const int64_t n = in->n;
+  out->n = n;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) {
+    GRPIC_CUDA_OK(cudaMemsetAsync(n_alive, 0, sizeof(int64_t), st));
+    return GRPIC_OK;
+  }
+  if (!ptc_args_ok(in) || !ptc_args_ok(out) || out->x1 == in->x1 || !tma_aligned(in) || n > 0xFFFFFFF0LL)
+    return GRPIC_ERR_ARG;
+  const size_t ntiles = (size_t)((n + 31) / 32);
+  const size_t need = (ntiles + ntiles / 2048 + 4096) * sizeof(uint32_t);
+  if (!ctx->ws || ctx->ws_bytes < need) return GRPIC_ERR_WORKSPACE;
+  uint32_t* offsets = (uint32_t*)ctx->ws;
+  tile_live_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in->flag, n, offsets);
+  int rc = grpic_exclusive_scan(offsets, ntiles, offsets + ntiles, st);
+  if (rc != GRPIC_OK) return rc;
+  rc = dispatch_push_deposit<true>(ctx, *in, *out, offsets, n_alive, *fields, *flux, dt, status, st);
+  if (rc != GRPIC_OK) return rc;
+  mark_tail_range_kernel<<<ctx->sm_count, 256, 0, st>>>(*out, n, n_alive);
+  grpic_count_launches(3);
+  return grpic_launch_ok();
 }

@@ -65,8 +65,9 @@ __global__ void __launch_bounds__(kThreads) scan_add_kernel(uint32_t* data, size
   for (int m = 0; m < 8; ++m)
     if (base + m < n) data[base + m] += off;
 }
+}  // namespace
 // In-place exclusive scan of data[0..n); scratch must hold >= n/2048 + n/2048^2 + 8 words.
-int exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st) {
+int grpic_exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st) {
   const size_t nb = (n + kScanTile - 1) / kScanTile;
   if (nb <= 1) {
     scan_tiles_kernel<<<1, kThreads, 0, st>>>(data, n, nullptr);
@@ -75,11 +76,12 @@ int exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st)
   }
   grpic_count_launches(2);
   scan_tiles_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
-  int rc = exclusive_scan(scratch, nb, scratch + nb, st);
+  int rc = grpic_exclusive_scan(scratch, nb, scratch + nb, st);
   if (rc != GRPIC_OK) return rc;
   scan_add_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
   return grpic_launch_ok();
 }
+namespace {
 
 // ------------------------------------------------------------------ radix sort passes
 __device__ __forceinline__ uint32_t make_key(uint32_t cell, uint32_t flag, uint32_t ncells) {
@@ -292,7 +294,7 @@ int grpic_sort(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, 
     } else {
       radix_hist_kernel<false><<<ntiles, kThreads, 0, st>>>(kin, nullptr, nullptr, n, ncells, shift, hist, ntiles);
     }
-    int rc = exclusive_scan(hist, nh, scratch, st);
+    int rc = grpic_exclusive_scan(hist, nh, scratch, st);
     if (rc != GRPIC_OK) return rc;
     if (p == 0) {
       radix_scatter_kernel<true><<<ntiles, kThreads, 0, st>>>(nullptr, nullptr, in->cell, in->flag, n, ncells,
@@ -326,7 +328,7 @@ int grpic_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* ou
   uint32_t* counts = (uint32_t*)ctx->ws;
   uint32_t* scratch = counts + ntiles;
   alive_count_kernel<<<ntiles, kThreads, 0, st>>>(in->flag, n, counts);
-  int rc = exclusive_scan(counts, ntiles, scratch, st);
+  int rc = grpic_exclusive_scan(counts, ntiles, scratch, st);
   if (rc != GRPIC_OK) return rc;
   compact_scatter_kernel<<<ntiles, kThreads, 0, st>>>(*in, *out, counts, ntiles, n_alive);
   mark_tail_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(*out, n, n_alive);

@@ -42,6 +42,7 @@ class CurrentC(C.Structure):
 
 EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_areas",
            "grpic_workspace_bytes", "grpic_set_workspace", "grpic_push_deposit",
+           "grpic_push_deposit_compact",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_sort", "grpic_compact", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
@@ -213,6 +214,15 @@ class Context:
         ps, fs, js = ptc.struct(), self._fields(fields), self._current(flux)
         _check(load().grpic_push_deposit(self.h, C.byref(ps), C.byref(fs), C.byref(js),
                                          C.c_double(dt), _ptr(self.status, _up), _stream()))
+
+    def push_deposit_compact(self, src, dst, fields, flux, dt, n_alive):
+        """compact(src -> dst) fused with push_deposit(dst); n_alive: int64 device tensor (1)."""
+        self.reserve(src.n)
+        a, b, fs, js = src.struct(), dst.struct(), self._fields(fields), self._current(flux)
+        _check(load().grpic_push_deposit_compact(
+            self.h, C.byref(a), C.byref(b), C.byref(fs), C.byref(js), C.c_double(dt),
+            C.cast(C.c_void_p(n_alive.data_ptr()), C.POINTER(C.c_int64)), _ptr(self.status, _up), _stream()))
+        dst.n = src.n
 
     def finalize_current(self, flux, filter_passes=0):
         js = self._current(flux)

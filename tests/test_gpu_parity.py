@@ -171,6 +171,49 @@ def test_axis_crossers_and_leavers(G, O):
         assert grid_err(Fref2[c], ctx.to_host(F2[c])) <= 1e-11, c
 
 
+@pytest.mark.parametrize("n,frac", [(0, 0.0), (31, 0.3), (5000, 0.0), (70001, 0.25), (4096, 1.0)])
+def test_push_deposit_compact_equals_compact_then_push(G, O, n, frac):
+    """grpic_push_deposit_compact == oracle compact -> oracle push+deposit: survivor order and
+    count bit-exact, x,u <= 1e-12, fluxes <= 1e-11, tail marked removed, input untouched."""
+    p = inputs.grid_params(64, 48, 0.99)
+    dt = inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "wald")
+    ptc = inputs.make_particles(p, max(n, 1), 21, "crowded", ("loguniform", 0.1, 1e3))
+    ptc = {k: v[:n].copy() for k, v in ptc.items()}
+    rng = np.random.default_rng(n + 1)
+    dead = rng.uniform(size=n) < frac
+    ptc["flag"] = (ptc["flag"] | np.where(dead, 2, 0)).astype(np.uint32)
+    keep = O.compact(ptc["flag"]) if n else np.zeros(0, np.int64)
+    assert len(keep) == int((~dead).sum())
+    sub = {k: np.ascontiguousarray(v[keep]) for k, v in ptc.items()}
+    ctx = G.Context(p, max(n, 1))
+    f_t = [ctx.to_device(f) for f in fields]
+    src, dst = G.Particles.from_numpy(ptc), G.Particles(n)
+    for t in dst.t.values():
+        t.fill_(7)
+    F_t = ctx.zeros(3)
+    n_alive = torch.full((1,), -1, dtype=torch.int64, device="cuda")
+    ctx.push_deposit_compact(src, dst, f_t, F_t, dt, n_alive)
+    torch.cuda.synchronize()
+    m = int(n_alive.item())
+    assert m == len(keep)
+    back = src.to_numpy()
+    for k in ptc:
+        assert np.array_equal(back[k], ptc[k]), k            # input not modified
+    got = dst.to_numpy()
+    if n:
+        assert np.all(got["flag"][m:] & 2) and np.all(got["cell"][m:] == 0xFFFFFFFF)
+    if m == 0:
+        assert all(float(F.abs().max()) == 0.0 for F in F_t)
+        return
+    ref, Fref = oracle_push_deposit(O, p, fields, sub, dt)
+    head = {k: v[:m] for k, v in got.items()}
+    check_push(p, sub, ref, head, O, fields, dt, max_frac=1e-3)
+    assert np.array_equal(head["w"], sub["w"])
+    for c in range(3):
+        assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
+
+
 def test_continuity_residual_gpu(G, O):
     """Charge conservation of the CUDA path itself: (rho1 - rho0) dV/dt + div F = 0 node by
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
