@@ -14,13 +14,13 @@
 //      guard copies and (last sweep) the damping layer in the epilogue.
 // No shared memory, no block barrier; lanes 2..29 of each warp produce output (halo 2+2).
 #include <math.h>
+#include <stdlib.h>
 
 #include "grpic_internal.cuh"
 
 namespace {
 
 constexpr int kOutCols = 28;   // output columns per warp
-constexpr int kRowChunk = 32;  // output rows per warp
 constexpr int kWarpsPerBlock = 4;
 
 struct SweepArgs {
@@ -32,6 +32,8 @@ struct SweepArgs {
   double* base_out[6];    // MODE 0: where to store the corrector base (may be null)
   double dt, a_impl, b_impl;
   int last;               // apply damping
+  int prefetch;           // software prefetch into L1 one row ahead
+  int row_chunk;          // output rows per warp (chosen per launch: one full wave of warps)
   int damp_cells;
   double damp_coef;
 };
@@ -42,11 +44,24 @@ struct Coef {  // at one staggered location
   double rho2;
   double s;
 };
+// 1/sqrt(x): MUFU.RSQ64H seed + two Newton steps (~1 ulp), no special-case path
+__device__ __forceinline__ double rsqrt_nr(double x) {
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+  const double h = 0.5 * x;
+  double e = fma(-(h * y), y, 0.5);
+  y = fma(y, e, y);
+  e = fma(-(h * y), y, 0.5);
+  return fma(y, e, y);
+}
+__device__ __forceinline__ void prefetch_l1(const double* p) {
+  asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
+}
 __device__ __forceinline__ Coef coef_at(const GridDev& g, double r, double s, double c) {
   Coef k;
   k.rho2 = fma(g.a2 * c, c, r * r);
   const double B = fma(2.0 * g.M, r, k.rho2);
-  const double rs = rsqrt(k.rho2 * B);
+  const double rs = rsqrt_nr(k.rho2 * B);
   k.al = k.rho2 * rs;
   k.q = B * rs;
   k.s = s;
@@ -68,15 +83,15 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0
 // the circulations themselves (diagnostics).
 template <int MODE>
 __global__ void __launch_bounds__(32 * kWarpsPerBlock)
-field_sweep_kernel(GridDev g, SweepArgs A) {
+field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs A) {
   const int lane = threadIdx.x & 31;
   const int wcol = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
   const int ibase = wcol * kOutCols;
   if (ibase > g.nr) return;
   const int i = ibase - 2 + lane;                       // this lane's column
   const int ic = min(max(i, -g.ng), g.nr + g.ng);       // clamped for loads
-  const int jstart = blockIdx.y * kRowChunk;
-  const int jend = min(jstart + kRowChunk, g.nth + 1);  // output rows [jstart, jend)
+  const int jstart = blockIdx.y * A.row_chunk;
+  const int jend = min(jstart + A.row_chunk, g.nth + 1);  // output rows [jstart, jend)
   const bool writer = (lane >= 2) && (lane < 2 + kOutCols) && (i <= g.nr);
 
   const double r_n = __ldg(g.r_n + ic + g.i0), r_h = __ldg(g.r_h + ic + g.i0);
@@ -92,6 +107,21 @@ field_sweep_kernel(GridDev g, SweepArgs A) {
     double Hph = 0, Hr = 0, Hth = 0, Eph = 0, Er = 0, Eth = 0;
     {
       const size_t k = g.idx(ic, jj);
+      if (A.prefetch) {
+        // next row of the iterate, and what the epilogue of THIS iteration reads (row jj-1)
+        if (jj < jend) {
+#pragma unroll
+          for (int c = 0; c < 6; ++c) prefetch_l1(A.in[c] + k + g.pitch);
+        }
+        if (jj > jstart && MODE != 2) {
+#pragma unroll
+          for (int c = 0; c < 6; ++c) prefetch_l1(A.base[c] + k - g.pitch);
+        }
+        if (jj > jstart) {
+          prefetch_l1(g.iADr + k - g.pitch); prefetch_l1(g.iADth + k - g.pitch); prefetch_l1(g.iADph + k - g.pitch);
+          prefetch_l1(g.iABr + k - g.pitch); prefetch_l1(g.iABth + k - g.pitch); prefetch_l1(g.iABph + k - g.pitch);
+        }
+      }
       const double Dr = __ldg(A.in[0] + k), Dth = __ldg(A.in[1] + k), Dph = __ldg(A.in[2] + k);
       const double Br = __ldg(A.in[3] + k), Bth = __ldg(A.in[4] + k), Bph = __ldg(A.in[5] + k);
       const double sn = __ldg(g.sin_n + jj + g.j0), cn = __ldg(g.cos_n + jj + g.j0);
@@ -242,10 +272,30 @@ int fill_guards(const GridDev& g, grpic_fields* f, cudaStream_t st) {
 }
 
 template <int MODE>
-int launch_sweep(const grpic_ctx* ctx, const SweepArgs& A, cudaStream_t st) {
+int launch_sweep(const grpic_ctx* ctx, SweepArgs A, cudaStream_t st) {
   const GridDev& g = ctx->g;
   const int wcols = (g.nr + 1 + kOutCols - 1) / kOutCols;
-  dim3 grid((wcols + kWarpsPerBlock - 1) / kWarpsPerBlock, (g.nth + 1 + kRowChunk - 1) / kRowChunk);
+  const int bcols = (wcols + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  // rows per warp: as many row chunks per column block as fill the resident CTAs exactly once
+  // (one full wave, every warp the same work), but at least 16 rows (2 halo rows per chunk)
+  static int per_sm = 0;
+  if (per_sm == 0) {
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, field_sweep_kernel<MODE>, 32 * kWarpsPerBlock,
+                                                      0) != cudaSuccess || per_sm < 1)
+      per_sm = 1;
+  }
+  static int max_rows = -1;
+  if (max_rows < 0) { const char* e = getenv("GRPIC_FS_MAXROWS"); max_rows = e ? atoi(e) : 32; }
+  const int resident = ctx->sm_count * per_sm;
+  const int nrows = g.nth + 1;
+  const int min_chunks = (nrows + max_rows - 1) / max_rows;
+  const int waves = (bcols * min_chunks + resident - 1) / resident;        // whole waves of CTAs
+  int chunks = waves * resident / bcols;
+  if (chunks < min_chunks) chunks = min_chunks;
+  int rows = (nrows + chunks - 1) / chunks;
+  if (rows < 16) rows = 16;
+  A.row_chunk = rows;
+  dim3 grid(bcols, (g.nth + 1 + rows - 1) / rows);
   field_sweep_kernel<MODE><<<grid, 32 * kWarpsPerBlock, 0, st>>>(g, A);
   grpic_count_launches(1);
   return grpic_launch_ok();
@@ -301,6 +351,9 @@ int grpic_field_step(grpic_ctx* ctx, grpic_fields* fields, const grpic_current* 
   if (rc != GRPIC_OK) return rc;
   const int N = ctx->p.field_iters;
   SweepArgs A = {};
+  static int pf = -1;
+  if (pf < 0) { const char* e = getenv("GRPIC_FS_PREFETCH"); pf = e ? atoi(e) : 1; }
+  A.prefetch = pf;
   A.dt = dt;
   A.b_impl = ctx->p.beta_impl;
   A.a_impl = 1.0 - ctx->p.beta_impl;
