@@ -9,7 +9,8 @@
  * Conventions
  *  - Every array argument is a CALLER-OWNED DEVICE pointer (cudaMalloc / torch CUDA tensor)
  *    unless it says "host".  The library never frees them and keeps no reference after the
- *    call returns, except the workspace registered with grpic_set_workspace.
+ *    call returns, except the workspace registered with grpic_set_workspace.  The context owns
+ *    its metric/area tables and (once grpic_step_host has been used) that call's staging buffers.
  *  - All work is enqueued on the caller's CUDA stream (`void* stream` = cudaStream_t; NULL =
  *    default stream) and is asynchronous; nothing synchronises the device.
  *  - Every call returns 0 on success or a negative grpic error code for argument / state
@@ -121,6 +122,23 @@ int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields*
 int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out,
                                const grpic_fields* fields, grpic_current* flux, double dt,
                                int64_t* n_alive, uint32_t* status, void* stream);
+
+/* END-TO-END step with the particle state in HOST memory (the one call that takes host
+ * pointers): host_ptc (HOST SoA; pinned memory makes the copies asynchronous), host_J (HOST,
+ * grid layout, nullable) and host_status (HOST word, nullable); `fields` / `background` stay
+ * DEVICE arrays.  Does, for one step: stream the particles through the GPU in chunks of
+ * `chunk_particles` (0 = 4 Mi) -- host->device copy, grpic_push_deposit_compact, device->host
+ * copy of the survivors, the three overlapped on separate streams -- then
+ * grpic_finalize_current and grpic_field_step on the device, and copies J back.  On return
+ * (the call BLOCKS until the host buffers are complete) host_ptc holds the survivors of the
+ * input, pushed one step, in their original order in entries [0, host_ptc->n) -- n is updated
+ * to the survivor count -- and `fields` is advanced one step.  The chunk staging buffers and the
+ * device flux arrays belong to the context (allocated on first use, freed by grpic_destroy);
+ * the workspace of grpic_field_step must be registered.  The step equals the device-resident
+ * sequence exactly, except for the summation order of the deposit. */
+int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_fields* fields,
+                    const grpic_fields* background, grpic_current* host_J, double dt,
+                    int32_t filter_passes, int64_t chunk_particles, uint32_t* host_status, void* stream);
 
 /* Fluxes -> current densities, in place: fold the theta ghost rows onto their mirror rows
  * (particles never cross the axis, :136), `filter_passes` passes of the (1,2,1)x(1,2,1)/16

@@ -148,6 +148,7 @@ int grpic_create(const grpic_params* p, grpic_ctx** out) {
   ctx->p = *p;
   ctx->ws = nullptr;
   ctx->ws_bytes = 0;
+  ctx->host_step = nullptr;
   cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
   GridDev& g = ctx->g;
   g.a = p->a; g.M = p->M; g.a2 = p->a * p->a; g.twoM = 2.0 * p->M;
@@ -201,6 +202,7 @@ int grpic_create(const grpic_params* p, grpic_ctx** out) {
 
 int grpic_destroy(grpic_ctx* ctx) {
   if (!ctx) return GRPIC_ERR_ARG;
+  grpic_host_step_release(ctx);
   cudaFree(ctx->tables);
   delete ctx;
   return GRPIC_OK;

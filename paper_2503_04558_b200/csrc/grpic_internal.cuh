@@ -37,6 +37,7 @@ struct grpic_ctx {
   void* ws;
   size_t ws_bytes;
   int sm_count;
+  void* host_step;  // staging buffers / streams of grpic_step_host (host_step.cu), lazily created
 };
 
 #define GRPIC_CUDA_OK(expr)                     \
@@ -60,3 +61,5 @@ __device__ __forceinline__ double ks_sqrtg(double a2, double M, double r, double
 void grpic_count_launches(int n);
 // in-place exclusive scan of data[0..n) (sort.cu); scratch >= n/2048 + n/2048^2 + 8 words
 int grpic_exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st);
+// frees the staging state of grpic_step_host (host_step.cu)
+void grpic_host_step_release(grpic_ctx* ctx);

@@ -42,7 +42,7 @@ class CurrentC(C.Structure):
 
 EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_areas",
            "grpic_workspace_bytes", "grpic_set_workspace", "grpic_push_deposit",
-           "grpic_push_deposit_compact",
+           "grpic_push_deposit_compact", "grpic_step_host",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_sort", "grpic_compact", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
@@ -223,6 +223,26 @@ class Context:
             self.h, C.byref(a), C.byref(b), C.byref(fs), C.byref(js), C.c_double(dt),
             C.cast(C.c_void_p(n_alive.data_ptr()), C.POINTER(C.c_int64)), _ptr(self.status, _up), _stream()))
         dst.n = src.n
+
+    def step_host(self, host, fields, dt, host_J=None, background=None, filter_passes=0, chunk=0):
+        """grpic_step_host: `host` = dict of (pinned) CPU torch tensors x1..u3, w, cell, flag and
+        "n" (int); updated in place, returns the survivor count."""
+        self.reserve(min(int(host["n"]), chunk or (4 << 20)))
+        ps = ParticlesC()
+        for k in PTC_F64:
+            setattr(ps, k, _ptr(host[k]))
+        for k in PTC_U32:
+            setattr(ps, k, _ptr(host[k], _up))
+        ps.n = int(host["n"])
+        fs = self._fields(fields)
+        bp = C.byref(self._fields(background)) if background is not None else None
+        jp = C.byref(self._current(host_J)) if host_J is not None else None
+        st = C.c_uint32(0)
+        _check(load().grpic_step_host(self.h, C.byref(ps), C.byref(fs), bp, jp, C.c_double(dt),
+                                      C.c_int32(filter_passes), C.c_int64(chunk), C.byref(st), _stream()))
+        host["n"] = int(ps.n)
+        self.last_host_status = st.value
+        return int(ps.n)
 
     def finalize_current(self, flux, filter_passes=0):
         js = self._current(flux)
