@@ -112,14 +112,13 @@ __device__ __forceinline__ void geodesic_rhs(const GridDev& g, const Pos& p, dou
 }
 
 // Generalised Boris, full dt (Eq.16-19).  D, B contravariant.
-__device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double sgn, double dt,
+__device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double alpha, double sgn, double dt,
                                       const double D[3], const double B[3], double& ur, double& ut,
                                       double& up) {
   const double s2 = p.s * p.s;
   const double g_rr = p.zp1, g_tt = p.rho2;
   const double g_rp = -g.a * s2 * p.zp1;
   const double g_pp = s2 * fma(g.a2 * s2, p.zp1, p.rho2);
-  const double alpha = p.h * rsqrt_nr(p.h);
   const double sqrtg = p.rho2 * p.s * p.zp1 * alpha;
   const double gu_rr = fma(p.r2a2, p.R, -p.beta), gu_tt = p.R, gu_pp = p.R * p.is2, gu_rp = g.a * p.R;
   const double hdt = sgn * dt * 0.5;
@@ -311,7 +310,10 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
                     const __grid_constant__ grpic_current J, double dt, int K, uint32_t* status) {
   __shared__ PtcTile tiles[kWarps][2];
   __shared__ __align__(8) uint64_t full[kWarps][2];
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  // read once (volatile: the compiler otherwise re-reads SR_TID.X, ~20 cycles each, when short of registers)
+  uint32_t tid_x;
+  asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
+  const int lane = tid_x & 31, warp = tid_x >> 5;
   const int tid = lane;                              // index inside the warp tile
   const int64_t ntiles = (ptc.n + 31) / 32;
   const int64_t tstride = (int64_t)gridDim.x * kWarps;
@@ -342,6 +344,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   __syncwarp();
 
   int it = 0;
+  uint32_t obase_next = (COMPACT && tile0 < ntiles) ? offsets[tile0] : 0u;   // loaded one tile ahead
   for (int64_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
   const int stage = it & 1;
   PtcTile& T = tiles[warp][stage];
@@ -366,7 +369,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   uint32_t live = 0, obase = 0;
   if (COMPACT) {
     live = __ballot_sync(0xffffffffu, active);
-    obase = offsets[tile];
+    obase = obase_next;
+    if (tnext < ntiles) obase_next = offsets[tnext];
     if (tile == ntiles - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
   }
 
@@ -401,10 +405,16 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     double s0, c0;
     sincos(x2, &s0, &c0);
     const Pos p0 = make_pos(g, r0, s0, c0);
+    const double alpha0 = p0.h * rsqrt_nr(p0.h);      // lapse at x^n
 
     double D[3], B[3];
     {
-      const double wxn = xa - fin, wyn = ya - fjn, wxh = xa - 0.5 - fih, wyh = ya - 0.5 - fjh;
+      double wxn = xa - fin;
+      // scheduling fence: the interpolation (first use of the 24 loads above) may not start
+      // before the position-only metric terms exist, so exp, sincos, the reciprocal and the
+      // rsqrt of the lapse all run in the shadow of the gather's L2 latency
+      asm volatile("" : "+d"(wxn) : "d"(p0.R), "d"(alpha0));
+      const double wyn = ya - fjn, wxh = xa - 0.5 - fih, wyh = ya - 0.5 - fjh;
       const double wx6[6] = {wxh, wxn, wxn, wxn, wxh, wxh};
       const double wy6[6] = {wyn, wyh, wyn, wyh, wyn, wyh};
       double V6[6];
@@ -419,7 +429,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 
     // ---- Boris (full dt) at x^n ----
     double ur = T.u1[tid], ut = T.u2[tid], up = T.u3[tid];
-    boris(g, p0, sgn, dt, D, B, ur, ut, up);
+    boris(g, p0, alpha0, sgn, dt, D, B, ur, ut, up);
 
     // ---- geodesic predictor + K correctors (Eq.14, 15) ----
     double Xr0, Xt0, Xp0, Ur0, Ut0;
@@ -534,8 +544,10 @@ template <bool COMPACT>
 int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
                           const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
                           const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
-  static int minb = -1;   // tuning knob (read once): resident CTAs per SM
-  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 5; }
+  // tuning knob (read once): resident CTAs per SM.  Measured at 1e8 particles: in place 7.11 ms
+  // (5 CTAs, 96 registers) vs 7.24 ms (4 CTAs); compacting 8.27 ms vs 7.80 ms
+  static int minb = -1;
+  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : (COMPACT ? 4 : 5); }
   if (ctx->p.geo_iters != 3)
     return launch_push_deposit<4, COMPACT, 0>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
   if (minb == 4)
