@@ -108,18 +108,18 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
     {
       const size_t k = g.idx(ic, jj);
       if (A.prefetch) {
-        // next row of the iterate, and what the epilogue of THIS iteration reads (row jj-1)
+        // next row of the iterate, and what the epilogue of the NEXT iteration reads (row jj)
         if (jj < jend) {
 #pragma unroll
           for (int c = 0; c < 6; ++c) prefetch_l1(A.in[c] + k + g.pitch);
         }
-        if (jj > jstart && MODE != 2) {
+        if (jj >= jstart && jj < jend) {
+          if (MODE != 2) {
 #pragma unroll
-          for (int c = 0; c < 6; ++c) prefetch_l1(A.base[c] + k - g.pitch);
-        }
-        if (jj > jstart) {
-          prefetch_l1(g.iADr + k - g.pitch); prefetch_l1(g.iADth + k - g.pitch); prefetch_l1(g.iADph + k - g.pitch);
-          prefetch_l1(g.iABr + k - g.pitch); prefetch_l1(g.iABth + k - g.pitch); prefetch_l1(g.iABph + k - g.pitch);
+            for (int c = 0; c < 6; ++c) prefetch_l1(A.base[c] + k);
+          }
+          prefetch_l1(g.iADr + k); prefetch_l1(g.iADth + k); prefetch_l1(g.iADph + k);
+          prefetch_l1(g.iABr + k); prefetch_l1(g.iABth + k); prefetch_l1(g.iABph + k);
         }
       }
       const double Dr = __ldg(A.in[0] + k), Dth = __ldg(A.in[1] + k), Dph = __ldg(A.in[2] + k);

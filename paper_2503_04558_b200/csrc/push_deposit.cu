@@ -555,12 +555,21 @@ int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, cons
   return launch_push_deposit<5, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
 }
 
-// live particles per 32-particle tile (one warp per tile, ballot)
+// live particles per 32-particle tile: each thread reads four flags (16 bytes), eight threads
+// cover a tile and add their counts by shuffles
 __global__ void __launch_bounds__(256) tile_live_kernel(const uint32_t* flag, int64_t n, uint32_t* counts) {
-  const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
-  const bool live = (k < n) && !(flag[k] & 2u);
-  const uint32_t b = __ballot_sync(0xffffffffu, live);
-  if ((threadIdx.x & 31) == 0 && k < n) counts[k >> 5] = __popc(b);
+  const int64_t k = ((int64_t)blockIdx.x * 256 + threadIdx.x) * 4;
+  uint32_t c = 0;
+  if (k + 4 <= n) {
+    const uint4 f = *reinterpret_cast<const uint4*>(flag + k);
+    c = !(f.x & 2u) + !(f.y & 2u) + !(f.z & 2u) + !(f.w & 2u);
+  } else {
+    for (int64_t q = k; q < n; ++q) c += !(flag[q] & 2u);
+  }
+  c += __shfl_xor_sync(0xffffffffu, c, 1);
+  c += __shfl_xor_sync(0xffffffffu, c, 2);
+  c += __shfl_xor_sync(0xffffffffu, c, 4);
+  if ((threadIdx.x & 7) == 0 && k < n) counts[k >> 5] = c;
 }
 // out[k] for k in [*n_alive, n): flag = removed
 __global__ void mark_tail_range_kernel(grpic_particles out, int64_t n, const int64_t* n_alive) {
@@ -616,7 +625,7 @@ extern "C" int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles*
   const size_t need = (ntiles + ntiles / 2048 + 4096) * sizeof(uint32_t);
   if (!ctx->ws || ctx->ws_bytes < need) return GRPIC_ERR_WORKSPACE;
   uint32_t* offsets = (uint32_t*)ctx->ws;
-  tile_live_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(in->flag, n, offsets);
+  tile_live_kernel<<<(unsigned)((n + 1023) / 1024), 256, 0, st>>>(in->flag, n, offsets);
   int rc = grpic_exclusive_scan(offsets, ntiles, offsets + ntiles, st);
   if (rc != GRPIC_OK) return rc;
   rc = dispatch_push_deposit<true>(ctx, *in, *out, offsets, n_alive, *fields, *flux, dt, status, st);
