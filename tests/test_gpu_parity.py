@@ -484,3 +484,67 @@ def test_config2_full_size_sampled(G, O):
     tot = (res + div)[Gd:Gd + nth + 1, Gd + 3:Gd + nr - 2]
     scale = np.max(np.abs(r1)) / dt
     assert np.max(np.abs(tot)) <= 1e-13 * scale, np.max(np.abs(tot)) / scale
+
+
+@pytest.mark.gpu
+def test_config3_full_size_bench_path(G, O):
+    """BASELINE.json config 3 at full size (2048^2, 1e8 particles) in the launch configuration
+    bench.py times: cell sort, then two fused push+deposit+compaction steps (the second one
+    squeezes out what the first removed).  Sort permutation vs the oracle's stable sort on the
+    whole set; a sample of particles pushed one by one by the oracle through both steps;
+    survivor counts and order bit-exact; flux moments at full size."""
+    cfg = inputs.config(3)
+    p, dt, fields, ptc = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    n = len(ptc["x1"])
+    ctx = G.Context(p, n)
+    f_t = [ctx.to_device(f) for f in fields]
+    A, B = G.Particles.from_numpy(ptc), G.Particles(n)
+    perm_t = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.sort(A, B, perm_t)
+    torch.cuda.synchronize()
+    perm = perm_t.cpu().numpy().view(np.uint32)
+    del perm_t
+    assert np.array_equal(perm, O.sort(ptc["cell"], ptc["flag"]))       # bit-exact at 1e8
+    n1 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    n2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    F1, F2 = ctx.zeros(3), ctx.zeros(3)
+    ctx.status.zero_()
+    ctx.push_deposit_compact(B, A, f_t, F1, dt, n1)                      # step 1: B -> A
+    torch.cuda.synchronize()
+    got1 = A.to_numpy()
+    assert int(n1.item()) == n and int(ctx.status.item()) == 0
+    ctx.push_deposit_compact(A, B, f_t, F2, dt, n2)                      # step 2: A -> B
+    torch.cuda.synchronize()
+    got2 = B.to_numpy()
+    alive1 = (got1["flag"] & 2) == 0
+    m2 = int(n2.item())
+    assert m2 == int(alive1.sum()) and m2 < n                            # some particles did leave
+    assert np.all(got2["flag"][m2:] & 2)
+    # oracle on a sample (particles are independent): positions in the sorted order
+    rng = np.random.default_rng(3)
+    sample = np.sort(rng.choice(n, 200_000, replace=False))
+    lost = np.flatnonzero(~alive1)
+    sample = np.union1d(sample, lost[:5000])                             # include leavers
+    src = perm[sample]
+    sub = {k: np.ascontiguousarray(v[src]) for k, v in ptc.items()}
+    ref1 = O.push(p, fields, sub, dt)
+    check_push(p, sub, ref1, {k: got1[k][sample] for k in got1}, O, fields, dt)
+    # step 2: survivors of the sample, at their compacted positions
+    pos2 = np.cumsum(alive1)[sample] - 1
+    keep = alive1[sample]
+    sub2 = {k: np.ascontiguousarray(got1[k][sample][keep]) for k in ("x1", "x2", "x3", "u1", "u2", "u3", "cell", "flag")}
+    # inputs of the oracle's second step are the ORACLE's own first-step outputs where they agree
+    # bit for bit in the integer fields; the float state is taken from the oracle
+    for k in ("x1", "x2", "x3", "u1", "u2", "u3"):
+        sub2[k] = np.ascontiguousarray(ref1[k][keep])
+    sub2["w"] = np.ascontiguousarray(sub["w"][keep])
+    ref2 = O.push(p, fields, sub2, dt)
+    g2 = {k: got2[k][pos2[keep]] for k in got2}
+    # the GPU's second step started from its own first-step state (<= 1e-12 from the oracle's):
+    # compare at 1e-11 (one more step of the same conditioning)
+    check_push(p, sub2, ref2, g2, O, fields, dt, tol=1e-11)
+    # flux moments of step 1 over all particles (properties that hold at any size)
+    Q = np.where(ptc["flag"][perm] & 1, 1.0, -1.0) * ptc["w"][perm]
+    dphi = got1["x3"] - ptc["x3"][perm]
+    Fph = ctx.to_host(F1[2])
+    assert abs(Fph.sum() - np.sum(Q * dphi) / dt) <= 1e-9 * np.sum(np.abs(Q * dphi)) / dt
