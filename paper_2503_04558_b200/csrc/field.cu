@@ -33,6 +33,7 @@ struct SweepArgs {
   double dt, a_impl, b_impl;
   int last;               // apply damping
   int prefetch;           // software prefetch into L1 one row ahead
+  int tma;                // stream the rows of interior warps through shared memory with bulk TMA copies
   int row_chunk;          // output rows per warp (chosen per launch: one full wave of warps)
   int damp_cells;
   double damp_coef;
@@ -53,6 +54,32 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
   y = fma(y, e, y);
   e = fma(-(h * y), y, 0.5);
   return fma(y, e, y);
+}
+// ---- bulk TMA (cp.async.bulk) + mbarrier plumbing ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  uint32_t ok;
+  do {
+    asm volatile(
+        "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
+        : "memory");
+  } while (!ok);
+}
+__device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(dst)),
+      "l"(src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
 }
 __device__ __forceinline__ void prefetch_l1(const double* p) {
   asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
@@ -81,18 +108,53 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0
 
 // MODE 0: predictor (Eq.9) + store corrector base; MODE 1: corrector (Eq.10); MODE 2: write
 // the circulations themselves (diagnostics).
-template <int MODE>
-__global__ void __launch_bounds__(32 * kWarpsPerBlock)
-field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs A) {
-  const int lane = threadIdx.x & 31;
-  const int wcol = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
-  const int ibase = wcol * kOutCols;
-  if (ibase > g.nr) return;
+// FAST: the warp's 28 output columns and its output rows lie strictly inside the physical
+// range of every component (no axis row, no first/last column): every range test, guard copy
+// and clamp folds away at compile time.  94 % of the warps of a 2048^2 sweep take this path.
+//
+// TMA (implies FAST): the warp streams its rows through a private two-stage ring in shared
+// memory.  A "packet" for iteration jj = the six iterate values of row jj, and the corrector
+// base + six area factors of row jj-1 (what that iteration's epilogue reads): 18 segments of
+// 32 doubles, each fetched by ONE 256-byte bulk TMA copy issued by lanes 0..17 in parallel and
+// signalled on the stage's mbarrier.  Packet jj+2 is requested as soon as packet jj is consumed,
+// so two rows are always in flight per warp without holding a register or an L1 line.
+constexpr int kSeg = 18;
+template <int MODE, bool FAST, bool TMA>
+__device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A, int lane, int ibase,
+                                           int jstart, int jend, double* ring, uint64_t* bars) {
   const int i = ibase - 2 + lane;                       // this lane's column
-  const int ic = min(max(i, -g.ng), g.nr + g.ng);       // clamped for loads
-  const int jstart = blockIdx.y * A.row_chunk;
-  const int jend = min(jstart + A.row_chunk, g.nth + 1);  // output rows [jstart, jend)
-  const bool writer = (lane >= 2) && (lane < 2 + kOutCols) && (i <= g.nr);
+  // ---- TMA plumbing: this lane's source array and row offset inside a packet ----
+  const double* myptr = nullptr;
+  if (TMA) {
+    const double* const areas[6] = {g.iADr, g.iADth, g.iADph, g.iABr, g.iABth, g.iABph};
+    if (lane < 6) myptr = A.in[lane];
+    else if (lane < 12) myptr = (MODE != 2) ? A.base[lane - 6] : nullptr;
+    else if (lane < kSeg) myptr = areas[lane - 12];
+  }
+  auto request = [&](int jj, int stage) {               // packet jj -> ring stage
+    if (jj > jend) return;
+    const bool epi = (jj - 1 >= jstart);                // epilogue operands of row jj-1 wanted
+    const uint32_t nseg = epi ? (MODE != 2 ? 18u : 12u) : 6u;
+    if (lane == 0) mbar_expect_tx(&bars[stage], nseg * 256u);
+    __syncwarp();
+    const bool mine = (lane < 6) || (epi && lane < kSeg && myptr != nullptr);
+    if (mine) {
+      const size_t k0 = g.idx(ibase - 2, lane < 6 ? jj : jj - 1);
+      tma_load_1d(ring + (stage * kSeg + lane) * 32, myptr + k0, 256u, &bars[stage]);
+    }
+  };
+  if (TMA) {
+    if (lane == 0) {
+      mbar_init(&bars[0], 1);
+      mbar_init(&bars[1], 1);
+      asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
+    request(jstart - 1, 0);
+    request(jstart, 1);
+  }
+  const int ic = FAST ? i : min(max(i, -g.ng), g.nr + g.ng);       // clamped for loads
+  const bool writer = (lane >= 2) && (lane < 2 + kOutCols) && (FAST || i <= g.nr);
 
   const double r_n = __ldg(g.r_n + ic + g.i0), r_h = __ldg(g.r_h + ic + g.i0);
   const double dr_n = __ldg(g.dr_n + ic + g.i0), dr_h = __ldg(g.dr_h + ic + g.i0);
@@ -105,25 +167,33 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
   for (int jj = jstart - 1; jj <= jend; ++jj) {
     // ---- auxiliary fields of row jj ----
     double Hph = 0, Hr = 0, Hth = 0, Eph = 0, Er = 0, Eth = 0;
+    const int nit = jj - (jstart - 1);
+    const double* rs = ring + ((nit & 1) * kSeg) * 32 + lane;      // this iteration's ring stage
     {
       const size_t k = g.idx(ic, jj);
-      if (A.prefetch) {
-        // next row of the iterate, and what the epilogue of the NEXT iteration reads (row jj)
-        if (jj < jend) {
+      if (!TMA && A.prefetch) {
+        // A.prefetch rows ahead: the iterate, and the operands of the epilogue (corrector base,
+        // area factors) of the row that far ahead
+        const int d = A.prefetch;
+        const size_t kp = k + (size_t)d * g.pitch;
+        if (jj + d <= jend) {
 #pragma unroll
-          for (int c = 0; c < 6; ++c) prefetch_l1(A.in[c] + k + g.pitch);
+          for (int c = 0; c < 6; ++c) prefetch_l1(A.in[c] + kp);
         }
-        if (jj >= jstart && jj < jend) {
+        if (jj + d - 1 >= jstart && jj + d - 1 < jend) {
+          const size_t ke = kp - g.pitch;
           if (MODE != 2) {
 #pragma unroll
-            for (int c = 0; c < 6; ++c) prefetch_l1(A.base[c] + k);
+            for (int c = 0; c < 6; ++c) prefetch_l1(A.base[c] + ke);
           }
-          prefetch_l1(g.iADr + k); prefetch_l1(g.iADth + k); prefetch_l1(g.iADph + k);
-          prefetch_l1(g.iABr + k); prefetch_l1(g.iABth + k); prefetch_l1(g.iABph + k);
+          prefetch_l1(g.iADr + ke); prefetch_l1(g.iADth + ke); prefetch_l1(g.iADph + ke);
+          prefetch_l1(g.iABr + ke); prefetch_l1(g.iABth + ke); prefetch_l1(g.iABph + ke);
         }
       }
-      const double Dr = __ldg(A.in[0] + k), Dth = __ldg(A.in[1] + k), Dph = __ldg(A.in[2] + k);
-      const double Br = __ldg(A.in[3] + k), Bth = __ldg(A.in[4] + k), Bph = __ldg(A.in[5] + k);
+      if (TMA) mbar_wait(&bars[nit & 1], (uint32_t)(nit >> 1) & 1u);
+      const double Dr = TMA ? rs[0] : __ldg(A.in[0] + k), Dth = TMA ? rs[32] : __ldg(A.in[1] + k);
+      const double Dph = TMA ? rs[64] : __ldg(A.in[2] + k), Br = TMA ? rs[96] : __ldg(A.in[3] + k);
+      const double Bth = TMA ? rs[128] : __ldg(A.in[4] + k), Bph = TMA ? rs[160] : __ldg(A.in[5] + k);
       const double sn = __ldg(g.sin_n + jj + g.j0), cn = __ldg(g.cos_n + jj + g.j0);
       const double sh = __ldg(g.sin_h + jj + g.j0), ch = __ldg(g.cos_h + jj + g.j0);
       const Coef knn = coef_at(g, r_n, sn, cn), khn = coef_at(g, r_h, sn, cn);
@@ -134,8 +204,8 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
       const double P7 = c_rphi(g, khn) * Dr, P8 = c_sgb(g, khn, r_h) * Bth;
       const double P1m = shfl_up1(P1), P6m = shfl_up1(P6), P7m = shfl_up1(P7), P8m = shfl_up1(P8);
       const double P2p = shfl_dn1(P2), P5p = shfl_dn1(P5), P3p = shfl_dn1(P3), P4p = shfl_dn1(P4);
-      const bool row_n = (jj >= 0) && (jj <= g.nth);      // node-in-theta rows
-      const bool row_h = (jj >= 0) && (jj <= g.nth - 1);  // half-in-theta rows
+      const bool row_n = FAST || ((jj >= 0) && (jj <= g.nth));      // node-in-theta rows
+      const bool row_h = FAST || ((jj >= 0) && (jj <= g.nth - 1));  // half-in-theta rows
       if (row_n) {
         Hth = fma(c_thth(khn), Bth, 0.5 * (P2 + P2p));                       // (B9)
         Er = fma(khn.q, Dr, 0.5 * (P5 + P5p));                               // (B11)
@@ -154,16 +224,19 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
     const int j = jj - 1;
     if (j >= jstart && writer) {
       const size_t k = g.idx(i, j);
-      const bool axis = (j == 0) || (j == g.nth);
-      const bool halfrow = (j < g.nth);
-      const bool halfcol = (i < g.nr);
+      const bool axis = !FAST && ((j == 0) || (j == g.nth));
+      const bool halfrow = FAST || (j < g.nth);
+      const bool halfcol = FAST || (i < g.nr);
       double C[6];
-      C[0] = (Hph_p - Hph_pp) * __ldg(g.iADr + k);                                    // (B8), Eq.(11) on the axes
-      C[1] = (Hph_im1_p - Hph_p) * __ldg(g.iADth + k);
-      C[2] = fma(Hth_p - Hth_im1_p, g.dth, (Hr_pp - Hr_p) * dr_n) * __ldg(g.iADph + k);
-      C[3] = -(Eph - Eph_p) * __ldg(g.iABr + k);                                      // (B10)
-      C[4] = -(Eph_p - Eph_ip1_p) * __ldg(g.iABth + k);
-      C[5] = -fma(Eth_ip1_p - Eth_p, g.dth, (Er_p - Er) * dr_h) * __ldg(g.iABph + k);
+      const double aDr = TMA ? rs[12 * 32] : __ldg(g.iADr + k), aDth = TMA ? rs[13 * 32] : __ldg(g.iADth + k);
+      const double aDph = TMA ? rs[14 * 32] : __ldg(g.iADph + k), aBr = TMA ? rs[15 * 32] : __ldg(g.iABr + k);
+      const double aBth = TMA ? rs[16 * 32] : __ldg(g.iABth + k), aBph = TMA ? rs[17 * 32] : __ldg(g.iABph + k);
+      C[0] = (Hph_p - Hph_pp) * aDr;                                                  // (B8), Eq.(11) on the axes
+      C[1] = (Hph_im1_p - Hph_p) * aDth;
+      C[2] = fma(Hth_p - Hth_im1_p, g.dth, (Hr_pp - Hr_p) * dr_n) * aDph;
+      C[3] = -(Eph - Eph_p) * aBr;                                                    // (B10)
+      C[4] = -(Eph_p - Eph_ip1_p) * aBth;
+      C[5] = -fma(Eth_ip1_p - Eth_p, g.dth, (Er_p - Er) * dr_h) * aBph;
       // physical range of each component
       const bool ok[6] = {halfcol, halfrow, !axis, halfrow, halfcol && !axis, halfcol && halfrow};
       // i of the last physical column of each component (for the radial guard copies)
@@ -183,21 +256,21 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
         if (MODE == 2) {
           v = ok[c] ? C[c] : 0.0;
         } else if (MODE == 0) {
-          const double Fn = __ldg(A.base[c] + k);
+          const double Fn = TMA ? rs[(6 + c) * 32] : __ldg(A.base[c] + k);
           const double Jc = (c < 3 && A.J[c]) ? __ldg(A.J[c] + k) : 0.0;
           v = ok[c] ? fma(A.dt, C[c] - Jc, Fn) : 0.0;
-          if (A.base_out[c] && rowok && i <= hi[c])
+          if (A.base_out[c] && rowok && (FAST || i <= hi[c]))
             A.base_out[c][k] = ok[c] ? fma(A.dt, A.a_impl * C[c] - Jc, Fn) : 0.0;
         } else {
-          v = ok[c] ? fma(A.dt * A.b_impl, C[c], __ldg(A.base[c] + k)) : 0.0;
+          v = ok[c] ? fma(A.dt * A.b_impl, C[c], TMA ? rs[(6 + c) * 32] : __ldg(A.base[c] + k)) : 0.0;
         }
         if (MODE != 2 && lam != 1.0 && ok[c]) {
           const double b = A.bg[c] ? __ldg(A.bg[c] + k) : 0.0;
           v = fma(v - b, lam, b);
         }
-        if (rowok && i <= hi[c]) {
+        if (rowok && (FAST || i <= hi[c])) {
           A.out[c][k] = v;
-          if (MODE != 2) {
+          if (MODE != 2 && !FAST) {
             if (i == 0)
               for (int gq = 1; gq <= g.ng; ++gq) A.out[c][k - gq] = v;
             if (i == hi[c])
@@ -206,11 +279,33 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
         }
       }
     }
+    if (TMA) {                                          // stage consumed: request the packet two rows on
+      __syncwarp();
+      request(jj + 2, nit & 1);
+    }
     // ---- rotate rows ----
     Hph_pp = Hph_p; Hr_pp = Hr_p;
     Hph_p = Hph; Hph_im1_p = Hph_im1; Hr_p = Hr; Hth_p = Hth; Hth_im1_p = Hth_im1;
     Eph_p = Eph; Eph_ip1_p = Eph_ip1; Er_p = Er; Eth_p = Eth; Eth_ip1_p = Eth_ip1;
   }
+}
+
+template <int MODE>
+__global__ void __launch_bounds__(32 * kWarpsPerBlock)
+field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs A) {
+  const int lane = threadIdx.x & 31;
+  const int wcol = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int ibase = wcol * kOutCols;
+  if (ibase > g.nr) return;
+  const int jstart = blockIdx.y * A.row_chunk;
+  const int jend = min(jstart + A.row_chunk, g.nth + 1);  // output rows [jstart, jend)
+  __shared__ __align__(128) double ring[kWarpsPerBlock][2 * kSeg * 32];
+  __shared__ __align__(8) uint64_t bars[kWarpsPerBlock][2];
+  const int w = threadIdx.x >> 5;
+  const bool fast = (ibase >= 1) && (ibase + kOutCols - 1 <= g.nr - 2) && (jstart >= 1) && (jend <= g.nth);
+  if (fast && A.tma) sweep_rows<MODE, true, true>(g, A, lane, ibase, jstart, jend, ring[w], bars[w]);
+  else if (fast) sweep_rows<MODE, true, false>(g, A, lane, ibase, jstart, jend, nullptr, nullptr);
+  else sweep_rows<MODE, false, false>(g, A, lane, ibase, jstart, jend, nullptr, nullptr);
 }
 
 // Axis values, radial guard copies and theta ghost rows by parity (S8); three tiny kernels.
@@ -354,6 +449,9 @@ int grpic_field_step(grpic_ctx* ctx, grpic_fields* fields, const grpic_current* 
   static int pf = -1;
   if (pf < 0) { const char* e = getenv("GRPIC_FS_PREFETCH"); pf = e ? atoi(e) : 1; }
   A.prefetch = pf;
+  static int tma = -1;
+  if (tma < 0) { const char* e = getenv("GRPIC_FS_TMA"); tma = e ? atoi(e) : 1; }
+  A.tma = tma;
   A.dt = dt;
   A.b_impl = ctx->p.beta_impl;
   A.a_impl = 1.0 - ctx->p.beta_impl;
