@@ -31,6 +31,7 @@ def build(force=False, verbose=False):
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
     flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
+    flags += os.environ.get("GRPIC_NVCC_EXTRA", "").split()
     if verbose:
         flags += ["-Xptxas", "-v"]
     cmd = [_nvcc()] + flags + ["-shared", "-o", LIB] + srcs

@@ -21,7 +21,14 @@
 namespace {
 
 constexpr int kOutCols = 28;   // output columns per warp
-constexpr int kWarpsPerBlock = 4;
+#ifndef GRPIC_FS_WARPS
+#define GRPIC_FS_WARPS 4
+#endif
+#ifndef GRPIC_FS_STAGES
+#define GRPIC_FS_STAGES 2
+#endif
+constexpr int kWarpsPerBlock = GRPIC_FS_WARPS;
+constexpr int kStages = GRPIC_FS_STAGES;   // ring depth of the TMA path (rows in flight per warp)
 
 struct SweepArgs {
   const double* in[6];    // iterate being evaluated (D^r,D^th,D^ph,B^r,B^th,B^ph)
@@ -112,12 +119,13 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0
 // range of every component (no axis row, no first/last column): every range test, guard copy
 // and clamp folds away at compile time.  94 % of the warps of a 2048^2 sweep take this path.
 //
-// TMA (implies FAST): the warp streams its rows through a private two-stage ring in shared
-// memory.  A "packet" for iteration jj = the six iterate values of row jj, and the corrector
+// TMA (implies FAST): the warp streams its rows through a private ring of stages in shared
+// memory (kStages deep).  A "packet" for iteration jj = the six iterate values of row jj, and the corrector
 // base + six area factors of row jj-1 (what that iteration's epilogue reads): 18 segments of
 // 32 doubles, each fetched by ONE 256-byte bulk TMA copy issued by lanes 0..17 in parallel and
-// signalled on the stage's mbarrier.  Packet jj+2 is requested as soon as packet jj is consumed,
-// so two rows are always in flight per warp without holding a register or an L1 line.
+// signalled on the stage's mbarrier.  Packet jj+kStages is requested as soon as packet jj is
+// consumed, so kStages rows are always in flight per warp without holding a register or an L1
+// line (measured: 2 stages x 4 warps per CTA is best; deeper rings cost occupancy).
 constexpr int kSeg = 18;
 template <int MODE, bool FAST, bool TMA>
 __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A, int lane, int ibase,
@@ -145,13 +153,13 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
   };
   if (TMA) {
     if (lane == 0) {
-      mbar_init(&bars[0], 1);
-      mbar_init(&bars[1], 1);
+#pragma unroll
+      for (int q = 0; q < kStages; ++q) mbar_init(&bars[q], 1);
       asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncwarp();
-    request(jstart - 1, 0);
-    request(jstart, 1);
+#pragma unroll
+    for (int q = 0; q < kStages; ++q) request(jstart - 1 + q, q);
   }
   const int ic = FAST ? i : min(max(i, -g.ng), g.nr + g.ng);       // clamped for loads
   const bool writer = (lane >= 2) && (lane < 2 + kOutCols) && (FAST || i <= g.nr);
@@ -168,7 +176,8 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
     // ---- auxiliary fields of row jj ----
     double Hph = 0, Hr = 0, Hth = 0, Eph = 0, Er = 0, Eth = 0;
     const int nit = jj - (jstart - 1);
-    const double* rs = ring + ((nit & 1) * kSeg) * 32 + lane;      // this iteration's ring stage
+    const int stg = nit % kStages;
+    const double* rs = ring + (stg * kSeg) * 32 + lane;            // this iteration's ring stage
     {
       const size_t k = g.idx(ic, jj);
       if (!TMA && A.prefetch) {
@@ -190,7 +199,7 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
           prefetch_l1(g.iABr + ke); prefetch_l1(g.iABth + ke); prefetch_l1(g.iABph + ke);
         }
       }
-      if (TMA) mbar_wait(&bars[nit & 1], (uint32_t)(nit >> 1) & 1u);
+      if (TMA) mbar_wait(&bars[stg], (uint32_t)(nit / kStages) & 1u);
       const double Dr = TMA ? rs[0] : __ldg(A.in[0] + k), Dth = TMA ? rs[32] : __ldg(A.in[1] + k);
       const double Dph = TMA ? rs[64] : __ldg(A.in[2] + k), Br = TMA ? rs[96] : __ldg(A.in[3] + k);
       const double Bth = TMA ? rs[128] : __ldg(A.in[4] + k), Bph = TMA ? rs[160] : __ldg(A.in[5] + k);
@@ -279,9 +288,9 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
         }
       }
     }
-    if (TMA) {                                          // stage consumed: request the packet two rows on
+    if (TMA) {                                          // stage consumed: request the packet kStages rows on
       __syncwarp();
-      request(jj + 2, nit & 1);
+      request(jj + kStages, stg);
     }
     // ---- rotate rows ----
     Hph_pp = Hph_p; Hr_pp = Hr_p;
@@ -299,8 +308,8 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
   if (ibase > g.nr) return;
   const int jstart = blockIdx.y * A.row_chunk;
   const int jend = min(jstart + A.row_chunk, g.nth + 1);  // output rows [jstart, jend)
-  __shared__ __align__(128) double ring[kWarpsPerBlock][2 * kSeg * 32];
-  __shared__ __align__(8) uint64_t bars[kWarpsPerBlock][2];
+  __shared__ __align__(128) double ring[kWarpsPerBlock][kStages * kSeg * 32];
+  __shared__ __align__(8) uint64_t bars[kWarpsPerBlock][kStages];
   const int w = threadIdx.x >> 5;
   const bool fast = (ibase >= 1) && (ibase + kOutCols - 1 <= g.nr - 2) && (jstart >= 1) && (jend <= g.nth);
   if (fast && A.tma) sweep_rows<MODE, true, true>(g, A, lane, ibase, jstart, jend, ring[w], bars[w]);
