@@ -541,7 +541,9 @@ void orc_geodesic_traj(double a, double M, int K, const double* y0, double dt, d
 // One particle step S4: gather D^n,B^n at x^n -> full-dt
 // Boris (PAPER.md:204 bundled half steps) -> geodesic -> x1 = ln r -> axis
 // reflection -> removal flag and new cell.
-// flag bit0: 1 = positron (q/m=+1), 0 = electron (q/m=-1); bit1: removed.
+// flag bit0: 1 = positron (q/m=+1), 0 = electron (q/m=-1); bit1: removed;
+// bit2: photon species (PAPER.md:153 "eps = 0 in u^0", :155 "photons ... only the geodesic
+// part"): no gather, no Boris, geodesic with eps = 0; carries no charge (no current, no rho).
 // x2dep = un-reflected new theta, used by the deposit (reading G13).
 // Particles whose removed bit is already set are copied through unchanged.
 void orc_push(const orc_params* p, const double* Dr, const double* Dth, const double* Dph,
@@ -559,22 +561,25 @@ void orc_push(const orc_params* p, const double* Dr, const double* Dth, const do
       x2dep[k] = x2[k]; celln[k] = 0xFFFFFFFFu; flagn[k] = flag[k];
       continue;
     }
+    const bool photon = (flag[k] & 4u) != 0;
     const double sgn = (flag[k] & 1u) ? 1.0 : -1.0;
     const double r = std::exp(x1[k]), th = x2[k];
-    const double fx = (x1[k] - g.xi_in) / g.dxi, fy = th / g.dth;
-    double D[3], B[3];
-    D[0] = gather1(g, Dr, ST_Dr, fx, fy);
-    D[1] = gather1(g, Dth, ST_Dth, fx, fy);
-    D[2] = gather1(g, Dph, ST_Dph, fx, fy);
-    B[0] = gather1(g, Br, ST_Br, fx, fy);
-    B[1] = gather1(g, Bth, ST_Bth, fx, fy);
-    B[2] = gather1(g, Bph, ST_Bph, fx, fy);
     const double u[3] = {u1[k], u2[k], u3[k]};
-    double ub[3];
-    boris(metric(g.a, g.M, r, th), u, D, B, sgn, dt, ub);
+    double ub[3] = {u[0], u[1], u[2]};
+    if (!photon) {
+      const double fx = (x1[k] - g.xi_in) / g.dxi, fy = th / g.dth;
+      double D[3], B[3];
+      D[0] = gather1(g, Dr, ST_Dr, fx, fy);
+      D[1] = gather1(g, Dth, ST_Dth, fx, fy);
+      D[2] = gather1(g, Dph, ST_Dph, fx, fy);
+      B[0] = gather1(g, Br, ST_Br, fx, fy);
+      B[1] = gather1(g, Bth, ST_Bth, fx, fy);
+      B[2] = gather1(g, Bph, ST_Bph, fx, fy);
+      boris(metric(g.a, g.M, r, th), u, D, B, sgn, dt, ub);
+    }
     const double y[6] = {r, th, x3[k], ub[0], ub[1], ub[2]};
     double yn[6];
-    geodesic(g.a, g.M, p->geo_iters, y, dt, 1.0, yn);
+    geodesic(g.a, g.M, p->geo_iters, y, dt, photon ? 0.0 : 1.0, yn);
     const double xi_new = std::log(yn[0]);
     double thn = yn[1], uth = yn[4];
     x2dep[k] = thn;
@@ -609,7 +614,7 @@ void orc_deposit(const orc_params* p, int64_t n, const double* x1o, const double
                  double* Fph) {
   const Grid g(*p);
   for (int64_t k = 0; k < n; ++k) {
-    if (flag[k] & 2u) continue;
+    if (flag[k] & (2u | 4u)) continue;                 // removed, or photon (no charge)
     const double Q = ((flag[k] & 1u) ? 1.0 : -1.0) * w[k];
     const double xa = (x1o[k] - g.xi_in) / g.dxi, xb = (x1n[k] - g.xi_in) / g.dxi;
     const double ya = x2o[k] / g.dth, yb = x2dep[k] / g.dth;
@@ -738,7 +743,7 @@ void orc_rho(const orc_params* p, int64_t n, const double* x1, const double* x2,
   const Grid g(*p);
   for (size_t k = 0; k < g.size(); ++k) rho[k] = 0.0;
   for (int64_t k = 0; k < n; ++k) {
-    if (flag[k] & 2u) continue;
+    if (flag[k] & (2u | 4u)) continue;                 // removed, or photon (no charge)
     const double Q = ((flag[k] & 1u) ? 1.0 : -1.0) * w[k];
     const double x = (x1[k] - g.xi_in) / g.dxi, y = x2[k] / g.dth;
     const int i0 = (int)std::floor(x), j0 = (int)std::floor(y);

@@ -285,3 +285,69 @@ def test_charged_orbit_conserves_eq24(name):
     e2, l2 = run(0.01, 20.0)
     assert e1 < 2e-3 and l1 < 2e-3
     assert 2.8 < e1 / e2 < 5.5 and 2.8 < l1 / l2 < 5.5, (e1, e2, l1, l2)
+
+
+# ------------------------------------------------------------------ photon species
+def test_photon_species_push_ignores_fields_and_moves_at_light_speed():
+    """flag bit2 = photon: no Lorentz force (identical result in any field), eps = 0 in u^0.
+    Flat space (M = 0): a photon follows a straight line at unit speed whatever |u| is
+    (closed form), and its energy |u| is conserved; pins eps = 0 (a massive particle with the
+    same u would move at |u|/sqrt(1+u^2) < 1)."""
+    from paper_2503_04558_b200 import inputs
+    p = inputs.grid_params(32, 32, 0.0, r_out=40.0, r_in=2.0, M=0.0)
+    strong = [np.full(inputs.grid_shape(p), 3.0) for _ in range(6)]
+    zero = [np.zeros(inputs.grid_shape(p)) for _ in range(6)]
+    n = 64
+    rng = np.random.default_rng(5)
+    r0 = rng.uniform(5.0, 20.0, n)
+    th0 = rng.uniform(0.5, 2.6, n)
+    # local orthonormal direction (e_r, e_theta, e_phi), |u| = p0
+    d = rng.normal(size=(n, 3)); d /= np.linalg.norm(d, axis=1)[:, None]
+    p0 = rng.uniform(0.05, 50.0, n)
+    ptc = dict(x1=np.log(r0), x2=th0.copy(), x3=np.zeros(n), u1=p0 * d[:, 0], u2=p0 * d[:, 1] * r0,
+               u3=p0 * d[:, 2] * r0 * np.sin(th0), w=np.ones(n),
+               flag=np.full(n, 4, np.uint32), cell=inputs.cells_of(p, np.log(r0), th0))
+    dt, steps = 0.01, 100
+    cur_a, cur_b = dict(ptc), dict(ptc)
+    for _ in range(steps):
+        na, nb = oracle.push(p, strong, cur_a, dt), oracle.push(p, zero, cur_b, dt)
+        for k in ("x1", "x2", "x3", "u1", "u2", "u3"):
+            assert np.array_equal(na[k], nb[k]), k                      # fields are not seen
+        cur_a = {**cur_a, **{k: na[k] for k in ("x1", "x2", "x3", "u1", "u2", "u3", "flag", "cell")}}
+        cur_b = {**cur_b, **{k: nb[k] for k in ("x1", "x2", "x3", "u1", "u2", "u3", "flag", "cell")}}
+    def cart(x1, x2, x3):
+        r = np.exp(x1)
+        return np.stack([r * np.sin(x2) * np.cos(x3), r * np.sin(x2) * np.sin(x3), r * np.cos(x2)], 1)
+    X0, X1 = cart(ptc["x1"], ptc["x2"], ptc["x3"]), cart(cur_a["x1"], cur_a["x2"], cur_a["x3"])
+    er = np.stack([np.sin(th0), np.zeros(n), np.cos(th0)], 1)
+    et = np.stack([np.cos(th0), np.zeros(n), -np.sin(th0)], 1)
+    ep = np.stack([np.zeros(n), np.ones(n), np.zeros(n)], 1)
+    dirc = d[:, :1] * er + d[:, 1:2] * et + d[:, 2:3] * ep
+    T = dt * steps
+    assert np.max(np.linalg.norm(X1 - (X0 + T * dirc), axis=1)) < 2e-4      # straight line, speed 1 (O(dt^2))
+    r1, t1 = np.exp(cur_a["x1"]), cur_a["x2"]
+    pmag = np.sqrt(cur_a["u1"] ** 2 + (cur_a["u2"] / r1) ** 2 + (cur_a["u3"] / (r1 * np.sin(t1))) ** 2)
+    assert np.max(np.abs(pmag / p0 - 1.0)) < 1e-5
+    # the same states as MASSIVE particles are slower: eps matters
+    mass = dict(ptc); mass["flag"] = np.zeros(n, np.uint32)
+    nm = oracle.push(p, zero, mass, dt)
+    v_m = np.linalg.norm(cart(nm["x1"], nm["x2"], nm["x3"]) - X0, axis=1) / dt
+    assert np.all(v_m < 1.0) and np.allclose(v_m, p0 / np.sqrt(1 + p0 ** 2), rtol=1e-3)
+
+
+def test_photons_carry_no_current_and_no_charge():
+    from paper_2503_04558_b200 import inputs
+    p = inputs.grid_params(24, 20, 0.9)
+    ptc = inputs.make_particles(p, 400, 3, "logical", ("loguniform", 0.1, 10.0))
+    fields = inputs.analytic_fields(p, "monopole")
+    dt = inputs.courant_dt(p)
+    ph = np.arange(400) % 3 == 0
+    mixed = dict(ptc); mixed["flag"] = (ptc["flag"] | np.where(ph, 4, 0)).astype(np.uint32)
+    new = oracle.push(p, fields, mixed, dt)
+    F = oracle.deposit(p, mixed, new, mixed["w"], dt)
+    sub = {k: np.ascontiguousarray(v[~ph]) for k, v in mixed.items()}
+    nsub = {k: np.ascontiguousarray(v[~ph]) for k, v in new.items()}
+    Fs = oracle.deposit(p, sub, nsub, sub["w"], dt)
+    for a, b in zip(F, Fs):
+        assert np.allclose(a, b, rtol=0, atol=1e-13 * max(1.0, np.max(np.abs(b))))
+    assert np.allclose(oracle.rho(p, mixed, mixed["w"]), oracle.rho(p, sub, sub["w"]), rtol=0, atol=1e-14)
