@@ -57,7 +57,9 @@ typedef struct {
  * both at integer time steps :176).  x1 = ln r, x2 = theta, x3 = phi.  w = macro-particle
  * weight.  cell = j*nr + i of the current position (0xFFFFFFFF once removed).
  * flag bit0: species sign, 1 = positron (q/m = +1), 0 = electron (q/m = -1);
- * flag bit1: removed (left through the inner or outer radial boundary). */
+ * flag bit1: removed (left through the inner or outer radial boundary);
+ * flag bit2: photon species: eps = 0 in u^0, no Lorentz force, no charge
+ * (pushed along null geodesics by the same calls; deposits nothing). */
 typedef struct {
   double *x1, *x2, *x3, *u1, *u2, *u3, *w;
   uint32_t *cell, *flag;

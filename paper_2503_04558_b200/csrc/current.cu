@@ -90,7 +90,7 @@ __global__ void rho_kernel(GridDev g, grpic_particles ptc, double* rho) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= ptc.n) return;
   const uint32_t flag = ptc.flag[k];
-  if (flag & 2u) return;
+  if (flag & (2u | 4u)) return;   // removed, or photon (no charge)
   const double Q = ((flag & 1u) ? 1.0 : -1.0) * ptc.w[k];
   const double x = (ptc.x1[k] - g.xi_in) * g.inv_dxi, y = ptc.x2[k] * g.inv_dth;
   const double fi = floor(x), fj = floor(y);

@@ -79,7 +79,8 @@ __device__ __forceinline__ Pos make_pos(const GridDev& g, double r, double s, do
 }
 
 // Right-hand sides X^i, U_i of Eq.(12) without the Lorentz force.
-__device__ __forceinline__ void geodesic_rhs(const GridDev& g, const Pos& p, double ur, double ut,
+// epsz = eps (1+z): eps = 1 for massive particles, 0 for photons.
+__device__ __forceinline__ void geodesic_rhs(const GridDev& g, const Pos& p, double epsz, double ur, double ut,
                                              double up, double& Xr, double& Xt, double& Xp,
                                              double& Ur, double& Ut) {
   const double R = p.R, R2 = R * R;
@@ -88,7 +89,7 @@ __device__ __forceinline__ void geodesic_rhs(const GridDev& g, const Pos& p, dou
   // P = rho^2 * (gamma^ij u_i u_j + beta u_r^2)
   const double P = fma(p.r2a2, ur2, fma(ut, ut, fma(2.0 * ur, aup, up2s)));
   const double N = fma(R, P, -p.beta * ur2);                 // gamma^ij u_i u_j
-  const double G2 = fma(N, p.zp1, p.zp1);                    // (u^0)^2 = (1+N)(1+z)
+  const double G2 = fma(N, p.zp1, epsz);                     // (u^0)^2 = (eps+N)(1+z)
   const double iu0 = rsqrt_nr(G2);
   const double u0 = G2 * iu0;
   const double Riu0 = R * iu0;
@@ -376,7 +377,10 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 
   if (active) {
     const double x1 = T.x1[tid], x2 = T.x2[tid];
-    const double sgn = (flag & 1u) ? 1.0 : -1.0;
+    // species: charge sign of e-/e+; a photon (bit2) feels no Lorentz force
+    // (sgn = 0 makes the Boris step the exact identity), has eps = 0 and carries no charge
+    const bool photon = (flag & 4u) != 0;
+    const double sgn = photon ? 0.0 : ((flag & 1u) ? 1.0 : -1.0);
 
     // ---- gather (first order, each component from its own staggered lattice): the 24
     // loads are issued first, exp / sincos / metric run while they are in flight ----
@@ -433,7 +437,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 
     // ---- geodesic predictor + K correctors (Eq.14, 15) ----
     double Xr0, Xt0, Xp0, Ur0, Ut0;
-    geodesic_rhs(g, p0, ur, ut, up, Xr0, Xt0, Xp0, Ur0, Ut0);
+    geodesic_rhs(g, p0, photon ? 0.0 : p0.zp1, ur, ut, up, Xr0, Xt0, Xp0, Ur0, Ut0);
     double dr = Xr0 * dt, dth = Xt0 * dt, dph = Xp0 * dt;      // increments from x^n
     double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
     const double hdt = 0.5 * dt;
@@ -445,7 +449,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       else sincos(x2 + dth, &s, &c);
       const Pos p1 = make_pos(g, r0 + dr, s, c);
       double Xr, Xt, Xp, Ur, Ut;
-      geodesic_rhs(g, p1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
+      geodesic_rhs(g, p1, photon ? 0.0 : p1.zp1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
       dr = hdt * (Xr + Xr0);
       dth = hdt * (Xt + Xt0);
       dph = hdt * (Xp + Xp0);
@@ -503,7 +507,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     dst.flag[kd] = nflag;
 
     // ---- deposit: 3x3 window anchored at the lower of the old / new cell ----
-    if (finite) {
+    if (finite && !photon) {
       const double q = sgn * T.w[tid];
       const double vph = q * dph * idt;
       const int ib = (int)floor(xb), jb = (int)floor(yb);

@@ -252,6 +252,28 @@ def test_step_host_matches_oracle_step(G, O, n, chunk):
         assert grid_err(fref[c], ctx.to_host(f_t[c])) <= 1e-11, c
 
 
+def test_photon_species_parity(G, O):
+    """mixed e-/e+/photon input (flag bit2 = photon): photons follow null
+    geodesics, ignore the fields and deposit nothing; same tolerances as the charged species."""
+    p = inputs.grid_params(64, 48, 0.99)
+    dt = inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "wald")
+    ptc = inputs.make_particles(p, 30000, 17, "crowded", ("loguniform", 0.1, 1e3))
+    ph = (np.arange(30000) % 3) == 0
+    ptc["flag"] = (ptc["flag"] | np.where(ph, 4, 0)).astype(np.uint32)
+    ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
+    ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
+    got = P.to_numpy()
+    check_push(p, ptc, ref, got, O, fields, dt, max_frac=1e-3)
+    assert np.array_equal(got["flag"] & 4, ptc["flag"] & 4)
+    for c in range(3):
+        assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
+    rho = ctx.zeros()
+    ctx.deposit_rho(P, rho)
+    alive = dict(ref); alive["w"] = ptc["w"]
+    assert grid_err(O.rho(p, alive, ptc["w"]), ctx.to_host(rho)) <= 1e-11
+
+
 def test_continuity_residual_gpu(G, O):
     """Charge conservation of the CUDA path itself: (rho1 - rho0) dV/dt + div F = 0 node by
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
