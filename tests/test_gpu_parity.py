@@ -452,6 +452,55 @@ def test_config1_ten_coupled_steps(G, O):
         assert grid_err(fo[c], ctx.to_host(f_t[c])) <= 1e-10, c
 
 
+def test_config5_coupled_loop_reduced(G, O):
+    """BASELINE.json config 5 recipe at reduced size (96^2, 40000 particles): 6 x (sort every 2
+    steps, fused push+deposit+removal, 3 binomial filter passes, field step N=7).  After every
+    step the particle ORDER and the integer state are compared bit for bit with the oracle loop
+    (stable sort, stable compaction), the float state at 1e-12 .. 1e-10 as the steps accumulate."""
+    cfg = inputs.config(5, nr=96, nth=96, n=40000)
+    p, dt, fields, ptc = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    ptc["w"][:] = 1e-6
+    n = len(ptc["x1"])
+    ctx = G.Context(p, n)
+    f_t = [ctx.to_device(f) for f in fields]
+    A, B = G.Particles.from_numpy(ptc), G.Particles(n)
+    n_alive = torch.zeros(1, dtype=torch.int64, device="cuda")
+    fo = [f.copy() for f in fields]
+    cur = dict(ptc)
+    keys = ("x1", "x2", "x3", "u1", "u2", "u3", "cell", "flag")
+    for step in range(6):
+        if step % 2 == 0:
+            perm = O.sort(cur["cell"], cur["flag"])
+            cur = {k: np.ascontiguousarray(v[perm]) for k, v in cur.items()}
+            ctx.sort(A, B)
+            A, B = B, A
+        keep = O.compact(cur["flag"])
+        cur = {k: np.ascontiguousarray(v[keep]) for k, v in cur.items()}
+        new, F = oracle_push_deposit(O, p, fo, cur, dt)
+        J = O.finalize_current(p, F, 3)
+        O.field_step(p, fo, J, dt)
+        w = cur["w"]
+        cur = {k: new[k] for k in keys}
+        cur["w"] = w
+        F_t = ctx.zeros(3)
+        ctx.push_deposit_compact(A, B, f_t, F_t, dt, n_alive)
+        A, B = B, A
+        ctx.finalize_current(F_t, 3)
+        ctx.field_step(f_t, F_t, dt)
+        torch.cuda.synchronize()
+        m = int(n_alive.item())
+        assert m == len(keep), (step, m, len(keep))
+        got = A.to_numpy(m)
+        tol = 1e-12 * 10 ** min(step, 2)
+        ex, eu = ptc_err(cur, got, ("x1", "x2", "x3")), ptc_err(cur, got, ("u1", "u2", "u3"))
+        assert (np.maximum(ex, eu) > tol).mean() < 1e-3, (step, (np.maximum(ex, eu) > tol).mean())
+        assert np.array_equal(got["flag"], cur["flag"]) and np.array_equal(got["cell"], cur["cell"]), step
+        for c in range(3):
+            assert grid_err(J[c], ctx.to_host(F_t[c])) <= 1e-10, (step, c)
+        for c in range(6):
+            assert grid_err(fo[c], ctx.to_host(f_t[c])) <= 1e-10, (step, c)
+
+
 def test_config2_full_size_sampled(G, O):
     """BASELINE.json config 2 at full size (1024^2, 2e7 particles) in the launch
     configuration bench.py times: sort, then one push+deposit step.  The oracle pushes a
