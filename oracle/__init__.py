@@ -54,6 +54,8 @@ def lib():
     if _lib is None:
         _lib = C.CDLL(build())
         _lib.orc_compact.restype = C.c_int64
+        _lib.orc_pair_production.restype = C.c_int64
+        _lib.orc_uniform.restype = C.c_double
         _lib.orc_num_threads.restype = C.c_int
     return _lib
 
@@ -233,6 +235,34 @@ def compact(flag):
     idx = np.zeros(n, dtype=np.uint32)
     c = lib().orc_compact(C.c_int64(n), _u(flag), _u(idx))
     return idx[:c].copy()
+
+
+def philox4x32_10(ctr, key):
+    c = (C.c_uint32 * 4)(*ctr); k = (C.c_uint32 * 2)(*key); o = (C.c_uint32 * 4)()
+    lib().orc_philox4x32_10(c, k, o)
+    return [int(v) for v in o]
+
+
+def uniform(seed, step, index):
+    return float(lib().orc_uniform(C.c_uint64(seed), C.c_uint32(step), C.c_uint64(index)))
+
+
+def pair_production(p, ptc, capacity, gamma_thr, eps_ph, p_convert, seed, step):
+    """one pass of the simplified pair production; returns (new particle
+    dict of the new length, overflow flag).  Input dict is not modified."""
+    n = len(ptc["x1"])
+    out = {}
+    for k, v in ptc.items():
+        a = np.zeros(capacity, dtype=v.dtype)
+        a[:n] = v
+        out[k] = a
+    ov = C.c_int32(0)
+    m = lib().orc_pair_production(C.byref(make_params(p)), C.c_int64(n), C.c_int64(capacity),
+                                  _d(out["x1"]), _d(out["x2"]), _d(out["x3"]), _d(out["u1"]), _d(out["u2"]),
+                                  _d(out["u3"]), _d(out["w"]), _u(out["cell"]), _u(out["flag"]),
+                                  C.c_double(gamma_thr), C.c_double(eps_ph), C.c_double(p_convert),
+                                  C.c_uint64(seed), C.c_uint32(step), C.byref(ov))
+    return {k: v[:m].copy() for k, v in out.items()}, bool(ov.value)
 
 
 def num_threads():

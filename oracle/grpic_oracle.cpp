@@ -20,6 +20,9 @@
 //   orc_circulation/field div B exactly preserved; div D - rho preserved; Wald/monopole
 //                         stationarity ~ Delta^2; Heun limit / order in dt
 //   orc_sort/orc_compact  = std::stable_sort / order-preserving filter (library definition)
+//   orc_philox4x32_10     the published known-answer vectors (tests/golden/philox4x32_10.txt)
+//   orc_pair_production   FIDO momentum / energy conservation, eps_ph, threshold, Eq.26 fraction,
+//                         append order; recoil and split prescriptions are readings P1-P4
 //   PARITY UNPINNED (paper silent; reading listed in DESIGN.md): field gather at
 //   staggered positions (G11/G12), damping profile (G14), current filter (S10),
 //   log-r basis choice (G8).
@@ -867,6 +870,89 @@ int64_t orc_compact(int64_t n, const uint32_t* flag, uint32_t* idx) {
   for (int64_t k = 0; k < n; ++k)
     if (!(flag[k] & 2u)) idx[c++] = (uint32_t)k;
   return c;
+}
+
+// ---------------------------------------------------------------------------
+// Simplified pair production of Section 4 (Eq.26).  Counter-based random
+// numbers: Philox4x32-10 (Salmon et al. 2011), written out from the published round function;
+// pinned by the known-answer vectors in tests/golden/philox4x32_10.txt.
+// ---------------------------------------------------------------------------
+void orc_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3], k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0, n1 = (uint32_t)p1;
+    const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1, n3 = (uint32_t)p0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+// uniform in [0,1) with 53 bits from the first two words; counter = (index lo, index hi, step, 0)
+double orc_uniform(uint64_t seed, uint32_t step, uint64_t index) {
+  const uint32_t ctr[4] = {(uint32_t)index, (uint32_t)(index >> 32), step, 0u};
+  const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
+  uint32_t o[4];
+  orc_philox4x32_10(ctr, key, o);
+  const uint64_t bits = (((uint64_t)o[0] << 32) | o[1]) >> 11;
+  return (double)bits * (1.0 / 9007199254740992.0);
+}
+
+// One pair-production pass over particles [0, n) (arrays have room for `capacity`), in the
+// paper's words plus the readings P1-P4 of DESIGN.md:
+//  * a lepton whose FIDO Lorentz factor Gamma = alpha u^0 = sqrt(1 + gamma^ij u_i u_j) reaches
+//    gamma_thr emits ONE photon of FIDO energy eps_ph "in the same direction": photon
+//    u_i = u_i eps_ph/|u| with |u| = sqrt(gamma^ij u_i u_j); the lepton keeps the rest of its
+//    momentum, u_i <- u_i (1 - eps_ph/|u|) (P1; only if |u| > eps_ph);
+//  * a photon converts with probability p_convert = 1 - exp(-tau dt) (Eq.26; the caller passes
+//    the number), decided by U(seed, step, index) < p_convert (P2); "each particle gets exactly
+//    half of the photon energy": E = |u| is the photon's FIDO energy now, each lepton gets
+//    Gamma = E/2 along the photon's direction, |u_l| = sqrt(Gamma^2 - 1) (P3; only if E/2 > 1).
+//    The photon's slot becomes the electron, the positron is a new particle;
+//  * new particles (photons, positrons) inherit position, cell and weight and are appended at
+//    n, n+1, ... in the order of their parents (P4).  Returns the new count (<= capacity;
+//    children beyond capacity are dropped and *overflow is set).
+int64_t orc_pair_production(const orc_params* p, int64_t n, int64_t capacity, double* x1, double* x2,
+                            double* x3, double* u1, double* u2, double* u3, double* w, uint32_t* cell,
+                            uint32_t* flag, double gamma_thr, double eps_ph, double p_convert,
+                            uint64_t seed, uint32_t step, int32_t* overflow) {
+  int64_t m = n;
+  *overflow = 0;
+  for (int64_t k = 0; k < n; ++k) {
+    if (flag[k] & 2u) continue;
+    const Metric g = metric(p->a, p->M, std::exp(x1[k]), x2[k]);
+    const double u[3] = {u1[k], u2[k], u3[k]};
+    const double N = norm_up(g, u);
+    double child_scale = 0.0, parent_scale = 1.0;
+    uint32_t child_flag = 0, parent_flag = flag[k];
+    if (!(flag[k] & 4u)) {                             // lepton: emission
+      const double Gamma = std::sqrt(1.0 + N), umag = std::sqrt(N);
+      if (Gamma >= gamma_thr && umag > eps_ph) {
+        child_scale = eps_ph / umag;
+        parent_scale = 1.0 - eps_ph / umag;
+        child_flag = 4u;
+      }
+    } else {                                           // photon: conversion
+      const double E = std::sqrt(N), Gl = 0.5 * E;
+      if (orc_uniform(seed, step, (uint64_t)k) < p_convert && Gl > 1.0) {
+        child_scale = parent_scale = std::sqrt(Gl * Gl - 1.0) / E;
+        parent_flag = 0u;                              // electron
+        child_flag = 1u;                               // positron
+      }
+    }
+    if (child_scale == 0.0) continue;
+    if (m < capacity) {
+      x1[m] = x1[k]; x2[m] = x2[k]; x3[m] = x3[k];
+      u1[m] = u[0] * child_scale; u2[m] = u[1] * child_scale; u3[m] = u[2] * child_scale;
+      w[m] = w[k]; cell[m] = cell[k]; flag[m] = child_flag;
+      ++m;
+    } else {
+      *overflow = 1;
+    }
+    u1[k] = u[0] * parent_scale; u2[k] = u[1] * parent_scale; u3[k] = u[2] * parent_scale;
+    flag[k] = parent_flag;
+  }
+  return m;
 }
 
 int orc_num_threads() {

@@ -351,3 +351,86 @@ def test_photons_carry_no_current_and_no_charge():
     for a, b in zip(F, Fs):
         assert np.allclose(a, b, rtol=0, atol=1e-13 * max(1.0, np.max(np.abs(b))))
     assert np.allclose(oracle.rho(p, mixed, mixed["w"]), oracle.rho(p, sub, sub["w"]), rtol=0, atol=1e-14)
+
+
+# ------------------------------------------------------------------ pair production (Eq.26)
+def test_philox_known_answers():
+    here = os.path.dirname(os.path.abspath(__file__))
+    rows = [l.split() for l in open(os.path.join(here, "golden", "philox4x32_10.txt")) if l[0] != "#"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        assert oracle.philox4x32_10(v[0:4], v[4:6]) == v[6:10]
+    u = np.array([oracle.uniform(7, 3, k) for k in range(20000)])
+    assert 0.0 <= u.min() and u.max() < 1.0
+    assert abs(u.mean() - 0.5) < 0.01 and abs(u.var() - 1.0 / 12.0) < 0.005
+    assert oracle.uniform(7, 3, 5) != oracle.uniform(7, 4, 5) != oracle.uniform(8, 3, 5)
+
+
+def _fido_norm(a, M, x1, x2, u1, u2, u3):
+    out = np.zeros(len(x1))
+    for k in range(len(x1)):
+        m = oracle.metric(a, M, math.exp(x1[k]), x2[k])
+        out[k] = (m["gu_rr"] * u1[k] ** 2 + m["gu_thth"] * u2[k] ** 2 + m["gu_phph"] * u3[k] ** 2
+                  + 2 * m["gu_rph"] * u1[k] * u3[k])
+    return out
+
+
+def test_pair_production_conserves_fido_momentum_and_energy():
+    """emission: photon + recoiling lepton carry the lepton's covariant momentum, the photon's FIDO
+    energy is eps_ph and only leptons with Gamma >= gamma_thr emit; conversion: a fraction
+    p_convert of the photons (Eq.26), the two leptons share the photon's FIDO energy, all momenta
+    parallel; children appended in parent order with position, cell and weight of the parent."""
+    from paper_2503_04558_b200 import inputs
+    p = inputs.grid_params(32, 32, 0.9)
+    n = 6000
+    ptc = inputs.make_particles(p, n, 9, "logical", ("loguniform", 1.0, 1e3))
+    ph = np.arange(n) % 2 == 1
+    ptc["flag"] = (ptc["flag"] | np.where(ph, 4, 0)).astype(np.uint32)
+    ptc["flag"][::50] |= 2                                    # some removed: untouched
+    ptc["w"] = np.random.default_rng(1).uniform(0.5, 2.0, n)
+    gthr, eph, pc = 100.0, 4.0, 0.3
+    out, ov = oracle.pair_production(p, ptc, 2 * n, gthr, eph, pc, seed=11, step=2)
+    assert not ov
+    m = len(out["x1"])
+    a, M = p["a"], p["M"]
+    N0 = _fido_norm(a, M, ptc["x1"], ptc["x2"], ptc["u1"], ptc["u2"], ptc["u3"])
+    live = (ptc["flag"] & 2) == 0
+    lep, pho = live & ~ph, live & ph
+    emit = lep & (np.sqrt(1 + N0) >= gthr) & (np.sqrt(N0) > eph)
+    assert 0 < emit.sum() < lep.sum()
+    changed = np.flatnonzero((out["u1"][:n] != ptc["u1"]) | (out["flag"][:n] != ptc["flag"]))
+    conv = np.zeros(n, bool); conv[changed] = True; conv &= pho
+    assert np.array_equal(np.flatnonzero(emit | conv), changed)       # nobody else was touched
+    assert m == n + len(changed)
+    # conversion decision = the stated uniform numbers, and the fraction is p_convert
+    U = np.array([oracle.uniform(11, 2, int(k)) for k in np.flatnonzero(pho)])
+    assert np.array_equal(np.flatnonzero(pho)[(U < pc) & (0.5 * np.sqrt(N0[pho]) > 1.0)], np.flatnonzero(conv))
+    assert abs(conv.sum() / pho.sum() - pc) < 4 * math.sqrt(pc * (1 - pc) / pho.sum())
+    # children in parent order, inheriting position, cell, weight
+    par = changed
+    for k in ("x1", "x2", "x3", "w", "cell"):
+        assert np.array_equal(out[k][n:], ptc[k][par]), k
+    U0 = np.stack([ptc["u1"], ptc["u2"], ptc["u3"]], 1)
+    Up = np.stack([out["u1"][:n], out["u2"][:n], out["u3"][:n]], 1)[par]
+    Uc = np.stack([out["u1"][n:], out["u2"][n:], out["u3"][n:]], 1)
+    Nc = _fido_norm(a, M, out["x1"][n:], out["x2"][n:], Uc[:, 0], Uc[:, 1], Uc[:, 2])
+    Np = _fido_norm(a, M, ptc["x1"][par], ptc["x2"][par], Up[:, 0], Up[:, 1], Up[:, 2])
+    e = emit[par]
+    # emission: momentum conserved, photon energy eps_ph, flags
+    assert np.allclose(Up[e] + Uc[e], U0[par][e], rtol=1e-13, atol=0)
+    assert np.allclose(np.sqrt(Nc[e]), eph, rtol=1e-12)
+    assert np.all(out["flag"][n:][e] == 4) and np.array_equal(out["flag"][:n][par][e], ptc["flag"][par][e])
+    # conversion: electron in the photon's slot, positron appended, each Gamma = E/2, parallel to the photon
+    c = ~e
+    E = np.sqrt(N0[par][c])
+    assert np.all(out["flag"][:n][par][c] == 0) and np.all(out["flag"][n:][c] == 1)
+    assert np.allclose(np.sqrt(1 + Np[c]), 0.5 * E, rtol=1e-12) and np.allclose(np.sqrt(1 + Nc[c]), 0.5 * E, rtol=1e-12)
+    assert np.array_equal(Up[c], Uc[c])
+    cosang = np.sum(Up[c] * U0[par][c], 1) / (np.linalg.norm(Up[c], axis=1) * np.linalg.norm(U0[par][c], axis=1))
+    assert np.allclose(cosang, 1.0, rtol=1e-12)
+    # capacity overflow is reported and nothing is written past it
+    out2, ov2 = oracle.pair_production(p, ptc, n + 5, gthr, eph, pc, seed=11, step=2)
+    assert ov2 and len(out2["x1"]) == n + 5
+    for k in out2:
+        assert np.array_equal(out2[k][n:], out[k][n:n + 5]), k
