@@ -79,6 +79,7 @@ enum {
 #define GRPIC_STATUS_FAR_MOVE 1u   /* a particle moved more than one cell in a step (still deposited exactly) */
 #define GRPIC_STATUS_NONFINITE 2u  /* a particle state became NaN/Inf (particle is flagged removed)           */
 #define GRPIC_STATUS_OFFGRID 4u    /* a deposit window left the guard region (contribution dropped)           */
+#define GRPIC_STATUS_CAPACITY 8u   /* grpic_pair_production created more particles than the arrays hold       */
 
 /* Create a context: validates params, computes on the device the area elements of Eq.(8)
  * (10-point Gauss-Legendre in xi and theta; D- and B-staggered sets) and
@@ -141,6 +142,30 @@ int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_
 int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_fields* fields,
                     const grpic_fields* background, grpic_current* host_J, double dt,
                     int32_t filter_passes, int64_t chunk_particles, uint32_t* host_status, void* stream);
+
+/* Simplified pair production of the paper's Section 4 (Eq.26), one pass over
+ * particles [0, ptc->n) of arrays that have room for `capacity` particles:
+ *  - a lepton whose FIDO Lorentz factor sqrt(1 + gamma^ij u_i u_j) >= gamma_thr (and whose
+ *    |u| = sqrt(gamma^ij u_i u_j) > eps_ph) emits one photon (flag bit2) of FIDO energy eps_ph
+ *    along its motion, u_i^ph = u_i eps_ph/|u|, and keeps u_i (1 - eps_ph/|u|);
+ *  - a photon converts with probability p_convert (= 1 - exp(-tau dt), Eq.26; the caller passes
+ *    the number), decided by the counter-based Philox4x32-10 uniform U(seed; index, step) <
+ *    p_convert, provided half its FIDO energy exceeds 1: its slot becomes the electron and a
+ *    positron is created, both with Lorentz factor E/2 along the photon's direction;
+ *  - created particles inherit position, cell and weight of their parent and are appended at
+ *    ptc->n, ptc->n + 1, ... in the order of their parents.
+ * The DEVICE word *n_new receives the new particle count (<= capacity; children beyond capacity
+ * are dropped and GRPIC_STATUS_CAPACITY is OR-ed into *status).  ptc->n is NOT changed by the
+ * call (the count is only known on the device).  Needs workspace (one word per 32 particles). */
+typedef struct {
+  double gamma_thr;   /* threshold FIDO Lorentz factor for emission (paper: 100)       */
+  double eps_ph;      /* FIDO energy of an emitted photon (paper: 4.0)                 */
+  double p_convert;   /* conversion probability per step, 1 - exp(-tau dt), in [0, 1]  */
+  uint64_t seed;      /* Philox key                                                    */
+  uint32_t step;      /* time-step counter (third counter word)                        */
+} grpic_pair_params;
+int grpic_pair_production(grpic_ctx* ctx, grpic_particles* ptc, int64_t capacity,
+                          const grpic_pair_params* params, int64_t* n_new, uint32_t* status, void* stream);
 
 /* Fluxes -> current densities, in place: fold the theta ghost rows onto their mirror rows
  * (particles never cross the axis, :136), `filter_passes` passes of the (1,2,1)x(1,2,1)/16

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgrpic.so")
-SOURCES = ["api.cu", "push_deposit.cu", "field.cu", "current.cu", "sort.cu", "host_step.cu"]
+SOURCES = ["api.cu", "push_deposit.cu", "field.cu", "current.cu", "sort.cu", "host_step.cu", "pair.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 

@@ -32,6 +32,11 @@ class ParticlesC(C.Structure):
                [("cell", _up), ("flag", _up), ("n", C.c_int64)]
 
 
+class PairParamsC(C.Structure):
+    _fields_ = [("gamma_thr", C.c_double), ("eps_ph", C.c_double), ("p_convert", C.c_double),
+                ("seed", C.c_uint64), ("step", C.c_uint32)]
+
+
 class FieldsC(C.Structure):
     _fields_ = [(k, _dp) for k in ("Dr", "Dth", "Dph", "Br", "Bth", "Bph")]
 
@@ -42,7 +47,7 @@ class CurrentC(C.Structure):
 
 EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_areas",
            "grpic_workspace_bytes", "grpic_set_workspace", "grpic_push_deposit",
-           "grpic_push_deposit_compact", "grpic_step_host",
+           "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_sort", "grpic_compact", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
@@ -243,6 +248,17 @@ class Context:
         host["n"] = int(ps.n)
         self.last_host_status = st.value
         return int(ps.n)
+
+    def pair_production(self, ptc, n, n_new, gamma_thr, eps_ph, p_convert, seed, step):
+        """grpic_pair_production on the first n entries of `ptc` (capacity = ptc.n);
+        n_new: int64 device tensor (1)."""
+        self.reserve(ptc.n)
+        ps = ptc.struct()
+        ps.n = int(n)
+        pp = PairParamsC(gamma_thr=gamma_thr, eps_ph=eps_ph, p_convert=p_convert, seed=seed, step=step)
+        _check(load().grpic_pair_production(
+            self.h, C.byref(ps), C.c_int64(ptc.n), C.byref(pp),
+            C.cast(C.c_void_p(n_new.data_ptr()), C.POINTER(C.c_int64)), _ptr(self.status, _up), _stream()))
 
     def finalize_current(self, flux, filter_passes=0):
         js = self._current(flux)
