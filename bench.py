@@ -45,6 +45,9 @@ UNIT = "particle-steps/s"
 # that `frac` equals the FP64 pipe utilisation ncu reports and is never flattered by it.
 FP64_INSTR_PER_PARTICLE = 689.0
 HBM_BYTES_PER_PARTICLE = 119.0
+# dram__bytes_read.sum + dram__bytes_write.sum of push_deposit_kernel<.,COMPACT> per live particle,
+# from the one `ncu --set full` capture of profiles/r01c (7.17 GB + 6.69 GB for 99.8e6 particles)
+NCU_DRAM_BYTES_PER_PARTICLE = 138.8
 # nominal FP64 pipe: 148 SMs x 64 DFMA lanes/clk x 1.965 GHz (B200)
 FP64_NOMINAL_INSTR_PER_S = 148 * 64 * 1.965e9
 
@@ -76,7 +79,7 @@ def parse():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -86,7 +89,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -293,7 +296,9 @@ def run_ours(args):
     roofline = {
         "kernel": "push_deposit_kernel", "bound": "alu" if t_alu >= t_hbm else "hbm",
         "achieved": 2.0 * fp64_ach / 1e12, "peak": 2.0 * fp64_peak_sust / 1e12, "unit": "TFLOP/s",
-        "frac": max(t_alu, t_hbm) / (pd_ms * 1e-3), "traffic": None,
+        "frac": max(t_alu, t_hbm) / (pd_ms * 1e-3),
+        "traffic": NCU_DRAM_BYTES_PER_PARTICLE * per_launch,
+        "traffic_source": "ncu --set full capture of profiles/r01c (bytes per particle) x particles per launch",
         "peak_source": "FP64 DFMA chain measured live on this device after the timed loop "
                        "(sustained clocks); 2 flop per FP64 pipe instruction",
         "peak_burst": 2.0 * fp64_peak_burst / 1e12,
