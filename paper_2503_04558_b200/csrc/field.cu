@@ -41,6 +41,7 @@ struct SweepArgs {
   int last;               // apply damping
   int prefetch;           // software prefetch into L1 one row ahead
   int tma;                // stream the rows of interior warps through shared memory with bulk TMA copies
+  int bcols, nchunks;     // CTA grid: column blocks x row chunks (linearised, edge blocks first)
   int row_chunk;          // output rows per warp (chosen per launch: one full wave of warps)
   int damp_cells;
   double damp_coef;
@@ -303,10 +304,19 @@ template <int MODE>
 __global__ void __launch_bounds__(32 * kWarpsPerBlock)
 field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs A) {
   const int lane = threadIdx.x & 31;
-  const int wcol = blockIdx.x * kWarpsPerBlock + (threadIdx.x >> 5);
+  // CTA order: the two edge column blocks of every row chunk first (their warps take the slower
+  // general path), then the interior blocks, so that no slow CTA ends up in the last wave
+  int bx, by;
+  {
+    const int id = blockIdx.x, edge = 2 * A.nchunks;
+    if (A.bcols < 3) { bx = id % A.bcols; by = id / A.bcols; }
+    else if (id < edge) { bx = (id & 1) ? A.bcols - 1 : 0; by = id >> 1; }
+    else { bx = 1 + (id - edge) % (A.bcols - 2); by = (id - edge) / (A.bcols - 2); }
+  }
+  const int wcol = bx * kWarpsPerBlock + (threadIdx.x >> 5);
   const int ibase = wcol * kOutCols;
   if (ibase > g.nr) return;
-  const int jstart = blockIdx.y * A.row_chunk;
+  const int jstart = by * A.row_chunk;
   const int jend = min(jstart + A.row_chunk, g.nth + 1);  // output rows [jstart, jend)
   __shared__ __align__(128) double ring[kWarpsPerBlock][kStages * kSeg * 32];
   __shared__ __align__(8) uint64_t bars[kWarpsPerBlock][kStages];
@@ -399,8 +409,9 @@ int launch_sweep(const grpic_ctx* ctx, SweepArgs A, cudaStream_t st) {
   int rows = (nrows + chunks - 1) / chunks;
   if (rows < 16) rows = 16;
   A.row_chunk = rows;
-  dim3 grid(bcols, (g.nth + 1 + rows - 1) / rows);
-  field_sweep_kernel<MODE><<<grid, 32 * kWarpsPerBlock, 0, st>>>(g, A);
+  A.bcols = bcols;
+  A.nchunks = (g.nth + 1 + rows - 1) / rows;
+  field_sweep_kernel<MODE><<<(unsigned)(A.bcols * A.nchunks), 32 * kWarpsPerBlock, 0, st>>>(g, A);
   grpic_count_launches(1);
   return grpic_launch_ok();
 }
