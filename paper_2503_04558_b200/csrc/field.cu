@@ -304,14 +304,16 @@ template <int MODE>
 __global__ void __launch_bounds__(32 * kWarpsPerBlock)
 field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ SweepArgs A) {
   const int lane = threadIdx.x & 31;
-  // CTA order: the two edge column blocks of every row chunk first (their warps take the slower
-  // general path), then the interior blocks, so that no slow CTA ends up in the last wave
+  // CTA order: the two edge column blocks of every row chunk and the two axis row chunks first
+  // (their warps take the slower general path), then the interior blocks, so that no slow CTA
+  // ends up in the last wave
   int bx, by;
   {
-    const int id = blockIdx.x, edge = 2 * A.nchunks;
-    if (A.bcols < 3) { bx = id % A.bcols; by = id / A.bcols; }
+    const int id = blockIdx.x, edge = 2 * A.nchunks, ic = A.bcols - 2, axis = 2 * ic;
+    if (A.bcols < 3 || A.nchunks < 3) { bx = id % A.bcols; by = id / A.bcols; }
     else if (id < edge) { bx = (id & 1) ? A.bcols - 1 : 0; by = id >> 1; }
-    else { bx = 1 + (id - edge) % (A.bcols - 2); by = (id - edge) / (A.bcols - 2); }
+    else if (id < edge + axis) { bx = 1 + (id - edge) % ic; by = ((id - edge) / ic) ? A.nchunks - 1 : 0; }
+    else { bx = 1 + (id - edge - axis) % ic; by = 1 + (id - edge - axis) / ic; }
   }
   const int wcol = bx * kWarpsPerBlock + (threadIdx.x >> 5);
   const int ibase = wcol * kOutCols;
