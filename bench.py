@@ -46,8 +46,8 @@ UNIT = "particle-steps/s"
 FP64_INSTR_PER_PARTICLE = 689.0
 HBM_BYTES_PER_PARTICLE = 119.0
 # dram__bytes_read.sum + dram__bytes_write.sum of push_deposit_kernel<.,COMPACT> per live particle,
-# from the one `ncu --set full` capture of profiles/r01c (7.17 GB + 6.69 GB for 99.8e6 particles)
-NCU_DRAM_BYTES_PER_PARTICLE = 138.8
+# from the one `ncu --set full` capture of profiles/r01e (6.52 GB + 6.52 GB for 99.8e6 particles)
+NCU_DRAM_BYTES_PER_PARTICLE = 130.7
 # nominal FP64 pipe: 148 SMs x 64 DFMA lanes/clk x 1.965 GHz (B200)
 FP64_NOMINAL_INSTR_PER_S = 148 * 64 * 1.965e9
 
@@ -79,7 +79,7 @@ def parse():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons sampled every 20 ms while the timed region runs."""
+    """nvidia-smi clocks / throttle reasons sampled every 50 ms while the timed region runs."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
@@ -89,7 +89,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "20"],
+                 "--format=csv,noheader,nounits", "-lms", "50"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -228,13 +228,13 @@ def run_ours(args):
             torch.cuda.synchronize()
 
     fp64_peak_burst = ctx.measure_fp64_peak()
+    sampler = ClockSampler(lrank) if rank == 0 else None    # started early: nvidia-smi needs ~0.2 s to begin
     state = (cur, alt)
     for s in range(W):
         state = step(s, state)
     barrier()
     setup_s = time.time() - t_setup
 
-    sampler = ClockSampler(lrank) if rank == 0 else None
     launches0 = ctx.kernel_launches()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -252,6 +252,8 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
     clocks = ClockSampler.summarise(sampler.window(tw0, tw1)) if sampler else None
+    if sampler:
+        sampler.stop()
 
     # particles actually pushed per timed step (alive at the start of the step)
     if compact:
@@ -298,7 +300,7 @@ def run_ours(args):
         "achieved": 2.0 * fp64_ach / 1e12, "peak": 2.0 * fp64_peak_sust / 1e12, "unit": "TFLOP/s",
         "frac": max(t_alu, t_hbm) / (pd_ms * 1e-3),
         "traffic": NCU_DRAM_BYTES_PER_PARTICLE * per_launch,
-        "traffic_source": "ncu --set full capture of profiles/r01c (bytes per particle) x particles per launch",
+        "traffic_source": "ncu --set full capture of profiles/r01e (bytes per particle) x particles per launch",
         "peak_source": "FP64 DFMA chain measured live on this device after the timed loop "
                        "(sustained clocks); 2 flop per FP64 pipe instruction",
         "peak_burst": 2.0 * fp64_peak_burst / 1e12,
