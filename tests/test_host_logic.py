@@ -106,3 +106,22 @@ def test_particle_sharding_two_ranks_gloo(tmp_path):
     outs = [p.communicate(timeout=300)[0].decode() for p in procs]
     assert all(p.returncode == 0 for p in procs), outs
     assert "OK" in outs[0]
+
+
+def test_bench_reference_arm_prints_contract_line():
+    """`bench.py --impl reference` (the oracle timed on the host cores) prints one JSON line with the
+    keys the driver reads; ranks other than 0 print nothing."""
+    import json
+    import subprocess
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1",
+           "--warmup", "1", "--particles", "3000", "--grid", "64"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=300, check=True).stdout.strip().splitlines()
+    d = json.loads(out[-1])
+    assert d["impl"] == "reference" and d["unit"] == "particle-steps/s" and d["value"] > 0
+    for k in ("metric", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+              "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert k in d, k
+    assert d["e2e"]["h2d_bytes_per_step"] == 0 and d["cpu_baseline"]["kind"] == "oracle"
+    env = dict(os.environ, RANK="1", WORLD_SIZE="2")
+    out1 = subprocess.run(cmd, capture_output=True, text=True, timeout=300, check=True, env=env).stdout.strip()
+    assert out1 == ""
