@@ -295,17 +295,19 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
 // One warp tile of particle input staged in shared memory (structure of arrays, 32 particles).
 constexpr int kWarps = kBlock / 32;
 struct __align__(128) PtcTile {
-  double x1[32], x2[32], x3[32], u1[32], u2[32], u3[32], w[32];
-  uint32_t flag[32];
+  double x1[kBlock], x2[kBlock], x3[kBlock], u1[kBlock], u2[kBlock], u3[kBlock], w[kBlock];
+  uint32_t flag[kBlock];
 };
-constexpr uint32_t kTileBytes = 7u * 32u * 8u + 32u * 4u;
+constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
 
-// Persistent kernel, warp-autonomous: every warp walks its own 32-particle tiles
-// (global warp id, + total warps, ...).  The particle state of a warp's NEXT tile is fetched by
-// eight 1-D bulk TMA copies into the warp's other shared-memory stage while the current tile
-// is pushed.  No block-wide barrier exists: a warp that takes a slow path (far deposit,
-// large-angle sincos) delays nobody.  The last, partial tile (n % 32 != 0) is staged
-// with plain loads.
+// Persistent kernel.  A CTA walks the 128-particle tiles blockIdx.x, + gridDim.x, ...; two
+// shared-memory stages hold the particle state of the current and the next tile, each filled by
+// eight 1-D bulk TMA copies (block-uniform addresses: no per-warp address arithmetic).  There is
+// no block-wide barrier in the loop: the four warps run independently, each waits on the
+// stage's mbarrier for its data, counts itself out of the stage when it has read it, and the
+// last warp out refills the stage with the tile two steps ahead.  A warp that takes a slow path
+// (far deposit, large-angle sincos) delays the others by at most one tile.  The last, partial
+// tile (n % 128 != 0) is staged with plain loads.
 //
 // COMPACT: the results are stored to `dst` at offsets[tile] + rank among the tile's live lanes
 // (offsets = exclusive scan of the per-tile live counts of `ptc`), i.e. particles already
@@ -317,53 +319,57 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
                     const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
                     int64_t* n_alive, const __grid_constant__ grpic_fields f,
                     const __grid_constant__ grpic_current J, double dt, int K, uint32_t* status) {
-  __shared__ PtcTile tiles[kWarps][2];
-  __shared__ __align__(8) uint64_t full[kWarps][2];
+  __shared__ PtcTile tiles[2];
+  __shared__ __align__(8) uint64_t full[2];
+  __shared__ uint32_t done[2];                       // warps that have finished reading a stage
   // read once (volatile: the compiler otherwise re-reads SR_TID.X, ~20 cycles each, when short of registers)
   uint32_t tid_x;
   asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
-  const int lane = tid_x & 31, warp = tid_x >> 5;
-  const int tid = lane;                              // index inside the warp tile
-  const int64_t ntiles = (ptc.n + 31) / 32;
-  const int64_t tstride = (int64_t)gridDim.x * kWarps;
+  const int tid = tid_x, lane = tid_x & 31, warp = tid_x >> 5;
+  const int64_t ntiles = (ptc.n + kBlock - 1) / kBlock;
+  const int64_t ntiles32 = (ptc.n + 31) / 32;         // COMPACT: offsets are per 32-particle tile
+  const int64_t tstride = gridDim.x;
   const double idt = 1.0 / dt;
 
   const uint64_t stream_policy = l2_evict_first_policy();
-  auto issue = [&](int64_t tile, int stage) {       // lane 0 only; full tiles only
-    const int64_t k0 = tile * 32;
-    if (k0 + 32 > ptc.n) return;
-    PtcTile& T = tiles[warp][stage];
-    uint64_t* bar = &full[warp][stage];
+  auto issue = [&](int64_t tile, int stage) {       // one thread; full tiles only
+    const int64_t k0 = tile * kBlock;
+    if (tile >= ntiles || k0 + kBlock > ptc.n) return;
+    PtcTile& T = tiles[stage];
+    uint64_t* bar = &full[stage];
     mbar_expect_tx(bar, kTileBytes);
-    tma_load_1d(T.x1, ptc.x1 + k0, 256, bar, stream_policy);
-    tma_load_1d(T.x2, ptc.x2 + k0, 256, bar, stream_policy);
-    tma_load_1d(T.x3, ptc.x3 + k0, 256, bar, stream_policy);
-    tma_load_1d(T.u1, ptc.u1 + k0, 256, bar, stream_policy);
-    tma_load_1d(T.u2, ptc.u2 + k0, 256, bar, stream_policy);
-    tma_load_1d(T.u3, ptc.u3 + k0, 256, bar, stream_policy);
-    tma_load_1d(T.w, ptc.w + k0, 256, bar, stream_policy);
-    tma_load_1d(T.flag, ptc.flag + k0, 128, bar, stream_policy);
+    tma_load_1d(T.x1, ptc.x1 + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.x2, ptc.x2 + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.x3, ptc.x3 + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.u1, ptc.u1 + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.u2, ptc.u2 + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.u3, ptc.u3 + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.w, ptc.w + k0, kBlock * 8, bar, stream_policy);
+    tma_load_1d(T.flag, ptc.flag + k0, kBlock * 4, bar, stream_policy);
   };
-  const int64_t tile0 = (int64_t)blockIdx.x * kWarps + warp;
-  if (lane == 0) {
-    mbar_init(&full[warp][0], 1);
-    mbar_init(&full[warp][1], 1);
+  const int64_t tile0 = blockIdx.x;
+  if (tid == 0) {
+    mbar_init(&full[0], 1);
+    mbar_init(&full[1], 1);
+    done[0] = 0;
+    done[1] = 0;
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    if (tile0 < ntiles) issue(tile0, 0);
+    issue(tile0, 0);
+    issue(tile0 + tstride, 1);
   }
-  __syncwarp();
+  __syncthreads();                                  // the only block barrier: before the loop
 
   int it = 0;
-  uint32_t obase_next = (COMPACT && tile0 < ntiles) ? offsets[tile0] : 0u;   // loaded one tile ahead
+  // COMPACT: output offset of this warp's 32-particle tile, loaded one tile ahead
+  uint32_t obase_next = (COMPACT && tile0 * kWarps + warp < ntiles32) ? offsets[tile0 * kWarps + warp] : 0u;
   for (int64_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
   const int stage = it & 1;
-  PtcTile& T = tiles[warp][stage];
-  const int64_t k = tile * 32 + lane;
-  const int64_t tnext = tile + tstride;
-  if (lane == 0 && tnext < ntiles) issue(tnext, stage ^ 1);
-  if (tile * 32 + 32 <= ptc.n) {
-    mbar_wait(&full[warp][stage], (uint32_t)(it >> 1) & 1u);
-  } else {                                          // partial last tile
+  PtcTile& T = tiles[stage];
+  const int64_t k = tile * kBlock + tid;
+  const int64_t tile32 = tile * kWarps + warp;      // this warp's 32-particle tile
+  if (tile * kBlock + kBlock <= ptc.n) {
+    mbar_wait(&full[stage], (uint32_t)(it >> 1) & 1u);
+  } else {                                          // partial last tile: every thread stages its own slot
     if (k < ptc.n) {
       T.x1[tid] = ptc.x1[k]; T.x2[tid] = ptc.x2[k]; T.x3[tid] = ptc.x3[k];
       T.u1[tid] = ptc.u1[k]; T.u2[tid] = ptc.u2[k]; T.u3[tid] = ptc.u3[k];
@@ -380,8 +386,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   if (COMPACT) {
     live = __ballot_sync(0xffffffffu, active);
     obase = obase_next;
-    if (tnext < ntiles) obase_next = offsets[tnext];
-    if (tile == ntiles - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
+    if (tile32 + tstride * kWarps < ntiles32) obase_next = offsets[tile32 + tstride * kWarps];
+    if (tile32 == ntiles32 - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
   }
 
   if (active) {
@@ -531,7 +537,14 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       }
     }
   }
-  __syncwarp();                                     // stage `stage` may be refilled next iteration
+  // this warp is done with the stage; the last warp out refills it with the tile two steps ahead
+  __syncwarp();
+  if (lane == 0) {
+    if (atomicAdd(&done[stage], 1u) == kWarps - 1) {
+      atomicExch(&done[stage], 0u);
+      issue(tile + 2 * tstride, stage);
+    }
+  }
   }
 }
 
@@ -557,8 +570,8 @@ template <bool COMPACT>
 int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
                           const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
                           const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
-  // tuning knob (read once): resident CTAs per SM.  Measured at 1e8 particles: in place 7.11 ms
-  // (5 CTAs, 96 registers) vs 7.24 ms (4 CTAs); compacting 8.27 ms vs 7.80 ms
+  // tuning knob (read once): resident CTAs per SM.  Measured at 1e8 particles: in place 6.65 ms
+  // (5 CTAs, 96 registers) vs 6.78 ms (4 CTAs); compacting 7.50 ms vs 7.16 ms
   static int minb = -1;
   if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : (COMPACT ? 4 : 5); }
   if (ctx->p.geo_iters != 3)
