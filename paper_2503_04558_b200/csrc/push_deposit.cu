@@ -274,6 +274,7 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         : "=r"(ok)
         : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
+    if (!ok) __nanosleep(64);                       // do not burn issue slots other warps can use
   } while (!ok);
 }
 // The particle stream (12.8 GB per step at 1e8) is read and written once: it is marked
@@ -294,18 +295,22 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
 
 // One warp tile of particle input staged in shared memory (structure of arrays, 32 particles).
 constexpr int kWarps = kBlock / 32;
+#ifndef GRPIC_PD_STAGES
+#define GRPIC_PD_STAGES 3
+#endif
+constexpr int kPdStages = GRPIC_PD_STAGES;   // particle tiles in flight per CTA
 struct __align__(128) PtcTile {
   double x1[kBlock], x2[kBlock], x3[kBlock], u1[kBlock], u2[kBlock], u3[kBlock], w[kBlock];
   uint32_t flag[kBlock];
 };
 constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
 
-// Persistent kernel.  A CTA walks the 128-particle tiles blockIdx.x, + gridDim.x, ...; two
-// shared-memory stages hold the particle state of the current and the next tile, each filled by
+// Persistent kernel.  A CTA walks the 128-particle tiles blockIdx.x, + gridDim.x, ...; a ring of
+// shared-memory stages holds the particle state of the current and the next tiles, each filled by
 // eight 1-D bulk TMA copies (block-uniform addresses: no per-warp address arithmetic).  There is
 // no block-wide barrier in the loop: the four warps run independently, each waits on the
 // stage's mbarrier for its data, counts itself out of the stage when it has read it, and the
-// last warp out refills the stage with the tile two steps ahead.  A warp that takes a slow path
+// last warp out refills the stage with the tile kPdStages steps ahead.  A warp that takes a slow path
 // (far deposit, large-angle sincos) delays the others by at most one tile.  The last, partial
 // tile (n % 128 != 0) is staged with plain loads.
 //
@@ -319,9 +324,9 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
                     const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
                     int64_t* n_alive, const __grid_constant__ grpic_fields f,
                     const __grid_constant__ grpic_current J, double dt, int K, uint32_t* status) {
-  __shared__ PtcTile tiles[2];
-  __shared__ __align__(8) uint64_t full[2];
-  __shared__ uint32_t done[2];                       // warps that have finished reading a stage
+  __shared__ PtcTile tiles[kPdStages];
+  __shared__ __align__(8) uint64_t full[kPdStages];
+  __shared__ uint32_t done[kPdStages];                       // warps that have finished reading a stage
   // read once (volatile: the compiler otherwise re-reads SR_TID.X, ~20 cycles each, when short of registers)
   uint32_t tid_x;
   asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
@@ -349,13 +354,11 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   };
   const int64_t tile0 = blockIdx.x;
   if (tid == 0) {
-    mbar_init(&full[0], 1);
-    mbar_init(&full[1], 1);
-    done[0] = 0;
-    done[1] = 0;
+#pragma unroll
+    for (int q = 0; q < kPdStages; ++q) { mbar_init(&full[q], 1); done[q] = 0; }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    issue(tile0, 0);
-    issue(tile0 + tstride, 1);
+#pragma unroll
+    for (int q = 0; q < kPdStages; ++q) issue(tile0 + q * tstride, q);
   }
   __syncthreads();                                  // the only block barrier: before the loop
 
@@ -363,12 +366,12 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   // COMPACT: output offset of this warp's 32-particle tile, loaded one tile ahead
   uint32_t obase_next = (COMPACT && tile0 * kWarps + warp < ntiles32) ? offsets[tile0 * kWarps + warp] : 0u;
   for (int64_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
-  const int stage = it & 1;
+  const int stage = it % kPdStages;
   PtcTile& T = tiles[stage];
   const int64_t k = tile * kBlock + tid;
   const int64_t tile32 = tile * kWarps + warp;      // this warp's 32-particle tile
   if (tile * kBlock + kBlock <= ptc.n) {
-    mbar_wait(&full[stage], (uint32_t)(it >> 1) & 1u);
+    mbar_wait(&full[stage], (uint32_t)(it / kPdStages) & 1u);
   } else {                                          // partial last tile: every thread stages its own slot
     if (k < ptc.n) {
       T.x1[tid] = ptc.x1[k]; T.x2[tid] = ptc.x2[k]; T.x3[tid] = ptc.x3[k];
@@ -542,7 +545,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   if (lane == 0) {
     if (atomicAdd(&done[stage], 1u) == kWarps - 1) {
       atomicExch(&done[stage], 0u);
-      issue(tile + 2 * tstride, stage);
+      issue(tile + kPdStages * tstride, stage);
     }
   }
   }
