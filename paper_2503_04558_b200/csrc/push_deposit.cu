@@ -205,17 +205,22 @@ __device__ __noinline__ void deposit_far(const GridDev* gp, double Q, double idt
 // Charge-conserving deposit of one move (Eq.21-23) on the 3x3-node window anchored at the
 // lower of the old and new cell in each direction: a move of less than one cell touches at
 // most two cells per direction, so 2 F_r faces x 3 rows, 3 columns x 2 F_theta faces and 3x3
-// F_phi nodes hold every non-zero flux.  xa, ya (old) and xb, yb (new) are window-relative
-// logical coordinates in [0,2].  No per-slot zero test (each costs a divergent branch around
-// the atomic); issuing all 21 REDs unconditionally is LSU-bound (12.5 ms vs 7.1 ms at 1e8).
+// F_phi nodes hold every non-zero flux.  Inputs per direction: the in-cell fractions of the old
+// and new position (fa, fb in [0,1)) and which of the window's two cells each lies in (oa, ob in
+// {0,1}).  The CIC shapes on the three nodes are then (1-f, f, 0) or (0, 1-f, f): plain selects,
+// no max() (a double fmax costs six instructions for its NaN rules).  No per-slot zero test (each
+// costs a divergent branch around the atomic); issuing all 21 REDs unconditionally is LSU-bound
+// (12.5 ms vs 7.1 ms at 1e8), so the slots that vanish unless a cell face is crossed are grouped.
 __device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t anchor, uint32_t pitch,
-                                              double Q, double vphi, double idt, double xa, double ya,
-                                              double xb, double yb, bool cx, bool cy) {
-  // CIC shapes on nodes 0,1,2:  S0 = max(0,1-x), S2 = max(0,x-1), S1 = 1-S0-S2
-  const double Sa0 = fmax(0.0, 1.0 - xa), Sa2 = fmax(0.0, xa - 1.0), Sa1 = (1.0 - Sa0) - Sa2;
-  const double Sb0 = fmax(0.0, 1.0 - xb), Sb2 = fmax(0.0, xb - 1.0), Sb1 = (1.0 - Sb0) - Sb2;
-  const double Ta0 = fmax(0.0, 1.0 - ya), Ta2 = fmax(0.0, ya - 1.0), Ta1 = (1.0 - Ta0) - Ta2;
-  const double Tb0 = fmax(0.0, 1.0 - yb), Tb2 = fmax(0.0, yb - 1.0), Tb1 = (1.0 - Tb0) - Tb2;
+                                              double Q, double vphi, double idt, double fxa, double fya,
+                                              double fxb, double fyb, bool oax, bool oay, bool obx,
+                                              bool oby) {
+  const double gxa = 1.0 - fxa, gya = 1.0 - fya, gxb = 1.0 - fxb, gyb = 1.0 - fyb;
+  const double Sa0 = oax ? 0.0 : gxa, Sa1 = oax ? gxa : fxa, Sa2 = oax ? fxa : 0.0;
+  const double Sb0 = obx ? 0.0 : gxb, Sb1 = obx ? gxb : fxb, Sb2 = obx ? fxb : 0.0;
+  const double Ta0 = oay ? 0.0 : gya, Ta1 = oay ? gya : fya, Ta2 = oay ? fya : 0.0;
+  const double Tb0 = oby ? 0.0 : gyb, Tb1 = oby ? gyb : fyb, Tb2 = oby ? fyb : 0.0;
+  const bool cx = oax != obx, cy = oay != oby;
   const double hq = -0.5 * Q * idt;
   // prefix sums of the shape differences over the two faces (Eq.21); the third vanishes
   const double Px0 = Sb0 - Sa0, Px1 = Sa2 - Sb2;
@@ -497,7 +502,11 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     const double th_dep = th;
     if (th < 0.0) { th = -th; vt = -vt; }
     if (th > M_PI) { th = 2.0 * M_PI - th; vt = -vt; }
+    // new logical position (un-reflected), its cell and in-cell fractions
     const double xb = (x1n - g.xi_in) * g.inv_dxi, yb = th_dep * g.inv_dth;
+    const double fib = floor(xb), fjb = floor(yb);
+    const int ib = (int)fib, jb = (int)fjb;
+    const double fxb = xb - fib, fyb = yb - fjb;
     uint32_t nflag = flag, ncell;
     const bool finite = isfinite(x1n) && isfinite(th) && isfinite(ph) && isfinite(vr) && isfinite(vt);
     const bool out = !finite || (x1n < g.xi_in) || (x1n >= g.xi_out);
@@ -508,10 +517,15 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     } else {
       // cell = floor of the quotient; the product form decides unless it is within 1e-7 of
       // a cell edge, where the quotient itself is taken (same decision as a division)
-      double cx = xb, cy = th * g.inv_dth;
-      if (fabs(cx - rint(cx)) < 1e-7) cx = (x1n - g.xi_in) / g.dxi;
-      if (fabs(cy - rint(cy)) < 1e-7) cy = th / g.dth;
-      int ic = (int)floor(cx), jc = (int)floor(cy);
+      int ic = ib, jc = jb;
+      if (fabs(fxb - 0.5) > 0.5 - 1e-7) ic = (int)floor((x1n - g.xi_in) / g.dxi);
+      if (th != th_dep) {                             // reflected at an axis: recompute in theta
+        const double cy = th * g.inv_dth, fc = floor(cy);
+        jc = (int)fc;
+        if (fabs(cy - fc - 0.5) > 0.5 - 1e-7) jc = (int)floor(th / g.dth);
+      } else if (fabs(fyb - 0.5) > 0.5 - 1e-7) {
+        jc = (int)floor(th / g.dth);
+      }
       ic = min(max(ic, 0), g.nr - 1);
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
@@ -528,13 +542,11 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     if (finite && !photon) {
       const double q = sgn * T.w[tid];
       const double vph = q * dph * idt;
-      const int ib = (int)floor(xb), jb = (int)floor(yb);
       const int di = ib - ia, dj = jb - ja;
       if (di >= -1 && di <= 1 && dj >= -1 && dj <= 1) {
         const int iw = min(ia, ib), jw = min(ja, jb);
-        const double ox = (double)iw, oy = (double)jw;
-        deposit_local(J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - ox,
-                               ya - oy, xb - ox, yb - oy, di != 0, dj != 0);
+        deposit_local(J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - fin, ya - fjn, fxb,
+                      fyb, ia != iw, ja != jw, ib != iw, jb != jw);
       } else {
         deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
       }
