@@ -336,15 +336,17 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   uint32_t tid_x;
   asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
   const int tid = tid_x, lane = tid_x & 31, warp = tid_x >> 5;
-  const int64_t ntiles = (ptc.n + kBlock - 1) / kBlock;
-  const int64_t ntiles32 = (ptc.n + 31) / 32;         // COMPACT: offsets are per 32-particle tile
-  const int64_t tstride = gridDim.x;
+  // all particle indices fit 32 bits (the C entry rejects n > 0xFFFFFFF0): one-instruction addressing
+  const uint32_t n32 = (uint32_t)ptc.n;
+  const uint32_t ntiles = (n32 + kBlock - 1) / kBlock;
+  const uint32_t ntiles32 = (n32 + 31) / 32;           // COMPACT: offsets are per 32-particle tile
+  const uint32_t tstride = gridDim.x;
   const double idt = 1.0 / dt;
 
   const uint64_t stream_policy = l2_evict_first_policy();
-  auto issue = [&](int64_t tile, int stage) {       // one thread; full tiles only
-    const int64_t k0 = tile * kBlock;
-    if (tile >= ntiles || k0 + kBlock > ptc.n) return;
+  auto issue = [&](uint32_t tile, int stage) {      // one thread; full tiles only
+    const uint32_t k0 = tile * kBlock;
+    if (tile >= ntiles || k0 + kBlock > n32) return;
     PtcTile& T = tiles[stage];
     uint64_t* bar = &full[stage];
     mbar_expect_tx(bar, kTileBytes);
@@ -357,7 +359,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     tma_load_1d(T.w, ptc.w + k0, kBlock * 8, bar, stream_policy);
     tma_load_1d(T.flag, ptc.flag + k0, kBlock * 4, bar, stream_policy);
   };
-  const int64_t tile0 = blockIdx.x;
+  const uint32_t tile0 = blockIdx.x;
   if (tid == 0) {
 #pragma unroll
     for (int q = 0; q < kPdStages; ++q) { mbar_init(&full[q], 1); done[q] = 0; }
@@ -370,15 +372,15 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   int it = 0;
   // COMPACT: output offset of this warp's 32-particle tile, loaded one tile ahead
   uint32_t obase_next = (COMPACT && tile0 * kWarps + warp < ntiles32) ? offsets[tile0 * kWarps + warp] : 0u;
-  for (int64_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
+  for (uint32_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
   const int stage = it % kPdStages;
   PtcTile& T = tiles[stage];
-  const int64_t k = tile * kBlock + tid;
-  const int64_t tile32 = tile * kWarps + warp;      // this warp's 32-particle tile
-  if (tile * kBlock + kBlock <= ptc.n) {
+  const uint32_t k = tile * kBlock + tid;
+  const uint32_t tile32 = tile * kWarps + warp;     // this warp's 32-particle tile
+  if (tile * kBlock + kBlock <= n32) {
     mbar_wait(&full[stage], (uint32_t)(it / kPdStages) & 1u);
   } else {                                          // partial last tile: every thread stages its own slot
-    if (k < ptc.n) {
+    if (k < n32) {
       T.x1[tid] = ptc.x1[k]; T.x2[tid] = ptc.x2[k]; T.x3[tid] = ptc.x3[k];
       T.u1[tid] = ptc.u1[k]; T.u2[tid] = ptc.u2[k]; T.u3[tid] = ptc.u3[k];
       T.w[tid] = ptc.w[k];
@@ -530,8 +532,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
     }
-    int64_t kd = k;
-    if (COMPACT) kd = (int64_t)obase + __popc(live & ((1u << lane) - 1u));
+    uint32_t kd = k;
+    if (COMPACT) kd = obase + __popc(live & ((1u << lane) - 1u));
     __stcs(dst.x1 + kd, x1n); __stcs(dst.x2 + kd, th); __stcs(dst.x3 + kd, ph);   // streaming stores
     __stcs(dst.u1 + kd, vr); __stcs(dst.u2 + kd, vt); __stcs(dst.u3 + kd, up);
     if (COMPACT) __stcs(dst.w + kd, T.w[tid]);
