@@ -55,6 +55,8 @@ struct Pos {          // position-only terms at (r, theta)
   double zp1;         // 1+z
   double h;           // 1/(1+z) = alpha^2
   double r2a2;        // r^2 + a^2
+  double r2;          // r^2
+  double sc2;         // 2 sin cos
 };
 
 __device__ __forceinline__ Pos make_pos(const GridDev& g, double r, double s, double c) {
@@ -75,6 +77,8 @@ __device__ __forceinline__ Pos make_pos(const GridDev& g, double r, double s, do
   p.h = p.rho2 * iB;
   p.zp1 = B * p.R;
   p.r2a2 = r2 + g.a2;
+  p.r2 = r2;
+  p.sc2 = (s + s) * c;
   return p;
 }
 
@@ -97,16 +101,17 @@ __device__ __forceinline__ void geodesic_rhs(const GridDev& g, const Pos& p, dou
   Xr = fma(fma(p.r2a2, ur, aup), Riu0, -p.beta * fma(ur, iu0, 1.0));
   Xt = Riu0 * ut;
   Xp = Riu0 * fma(up, p.is2, g.a * ur);
-  // derivatives: dz/dr = 2M (a^2 c^2 - r^2)/rho^4, dz/dth = 4 M r a^2 s c / rho^4; W = 1/(1+z)^2
-  const double A = g.a2 * p.s * p.c;
+  // derivatives: dz/dr = 2M (a^2 c^2 - r^2)/rho^4, dz/dth = 4 M r a^2 s c / rho^4; W = 1/(1+z)^2;
+  // a^2 c^2 - r^2 = rho^2 - 2 r^2
+  const double A2 = g.a2 * p.sc2;                            // 2 a^2 sin cos
   const double WR2 = p.h * p.h * R2 * g.twoM;
-  const double Wdzr = WR2 * fma(g.a2 * p.c, p.c, -p.r * p.r);
-  const double Wdzt = WR2 * 2.0 * p.r * A;
+  const double Wdzr = WR2 * fma(-2.0, p.r2, p.rho2);
+  const double Wdzt = (WR2 * p.r) * A2;
   const double lead = fma(0.5, u0, ur);                      // (u^0/2 + u_r)
   // (d_i gamma^jk) u_j u_k
   const double twor = p.r + p.r;
   const double quad_r = fma(-twor * R2, P, (twor * R - Wdzr) * ur2);
-  const double quad_t = fma(2.0 * A * R2, P, -fma(2.0 * R * p.c * p.is2 * p.s, up2s, Wdzt * ur2));
+  const double quad_t = fma(A2 * R2, P, -fma((R * p.is2) * p.sc2, up2s, Wdzt * ur2));
   const double hiu0 = 0.5 * iu0;
   Ur = fma(Wdzr, lead, -quad_r * hiu0);
   Ut = fma(Wdzt, lead, -quad_t * hiu0);
