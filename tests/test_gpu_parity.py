@@ -312,6 +312,30 @@ def test_pair_production_parity(G, O, n, cap, step):
         assert err.max(initial=0.0) <= 1e-12, (k, err.max())
 
 
+def test_far_moves_take_the_general_window(G, O):
+    """dt three times the Courant-limited step: fast particles move more than one cell, leave the
+    3x3 window and must take the exact general-window deposit (GRPIC_STATUS_FAR_MOVE is set);
+    fluxes still match the oracle, which deposits on whatever window the move spans."""
+    p = inputs.grid_params(64, 64, 0.9, r_out=30.0)
+    dt = 6.0 * inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "monopole")
+    ptc = inputs.make_particles(p, 20000, 13, "logical", ("loguniform", 5.0, 100.0))
+    dxi, dth = inputs.spacing(p)
+    inner = (ptc["x1"] > p["xi_in"] + 8 * dxi) & (ptc["x1"] < p["xi_out"] - 8 * dxi) & \
+            (ptc["x2"] > 8 * dth) & (ptc["x2"] < np.pi - 8 * dth)
+    ptc = {k: np.ascontiguousarray(v[inner]) for k, v in ptc.items()}
+    ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
+    far = (np.abs(np.floor((ref["x1"] - p["xi_in"]) / dxi) - np.floor((ptc["x1"] - p["xi_in"]) / dxi)) > 1) | \
+          (np.abs(np.floor(ref["x2dep"] / dth) - np.floor(ptc["x2"] / dth)) > 1)
+    assert far.sum() > 100
+    ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
+    st = int(ctx.status.item())
+    assert st & 1 and not (st & ~1)
+    check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-3)
+    for c in range(3):
+        assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
+
+
 def test_continuity_residual_gpu(G, O):
     """Charge conservation of the CUDA path itself: (rho1 - rho0) dV/dt + div F = 0 node by
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
