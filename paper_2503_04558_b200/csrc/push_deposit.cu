@@ -397,12 +397,13 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   }
   const uint32_t flag = T.flag[tid];
   const bool active = !(flag & 2u);
-  uint32_t live = 0, obase = 0;
+  uint32_t kd = k;                                   // where this particle's result is stored
   if (COMPACT) {
-    live = __ballot_sync(0xffffffffu, active);
-    obase = obase_next;
+    const uint32_t live = __ballot_sync(0xffffffffu, active);
+    const uint32_t obase = obase_next;
     if (tile32 + tstride * kWarps < ntiles32) obase_next = offsets[tile32 + tstride * kWarps];
     if (tile32 == ntiles32 - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
+    kd = obase + __popc(live & ((1u << lane) - 1u));
   }
 
   if (active) {
@@ -537,8 +538,6 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
     }
-    uint32_t kd = k;
-    if (COMPACT) kd = obase + __popc(live & ((1u << lane) - 1u));
     __stcs(dst.x1 + kd, x1n); __stcs(dst.x2 + kd, th); __stcs(dst.x3 + kd, ph);   // streaming stores
     __stcs(dst.u1 + kd, vr); __stcs(dst.u2 + kd, vt); __stcs(dst.u3 + kd, up);
     if (COMPACT) __stcs(dst.w + kd, T.w[tid]);
