@@ -157,17 +157,26 @@ __device__ __forceinline__ void red_add(double* p, double v) {
       "d"(v)
       : "memory");
 }
-// sin, cos of th0 + d from (s0, c0) for |d| <= 0.06 (angle addition, Taylor in d).
+// sin, cos of th0 + d from (s0, c0) for |d| <= 0.06 (angle addition, Taylor in d).  SHORT:
+// |d| <= 2^-9, where two terms less of each series are exact to < 1e-19 (the step of a particle
+// is dt X^theta <= dt / rho: at the production time steps every corrector takes this path).
+template <bool SHORT>
 __device__ __forceinline__ void sincos_shift(double s0, double c0, double d, double& s, double& c) {
   const double d2 = d * d;
-  double ps = fma(d2, 1.0 / 362880.0, -1.0 / 5040.0);
-  ps = fma(ps, d2, 1.0 / 120.0);
-  ps = fma(ps, d2, -1.0 / 6.0);
+  double ps, pc;
+  if (SHORT) {
+    ps = fma(d2, 1.0 / 120.0, -1.0 / 6.0);
+    pc = fma(fma(d2, 1.0 / 720.0, -1.0 / 24.0), d2, 0.5);
+  } else {
+    ps = fma(d2, 1.0 / 362880.0, -1.0 / 5040.0);
+    ps = fma(ps, d2, 1.0 / 120.0);
+    ps = fma(ps, d2, -1.0 / 6.0);
+    pc = fma(d2, 1.0 / 3628800.0, -1.0 / 40320.0);
+    pc = fma(pc, d2, 1.0 / 720.0);
+    pc = fma(pc, d2, -1.0 / 24.0);
+    pc = fma(pc, d2, 0.5);
+  }
   const double sd = fma(ps * d2, d, d);                         // sin d
-  double pc = fma(d2, 1.0 / 3628800.0, -1.0 / 40320.0);
-  pc = fma(pc, d2, 1.0 / 720.0);
-  pc = fma(pc, d2, -1.0 / 24.0);
-  pc = fma(pc, d2, 0.5);
   const double vd = pc * d2;                                    // 1 - cos d
   s = s0 + fma(c0, sd, -s0 * vd);
   c = c0 - fma(s0, sd, c0 * vd);
@@ -476,7 +485,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 #pragma unroll
     for (int ci = 0; ci < KK; ++ci) {
       double s, c;
-      if (fabs(dth) <= 0.06) sincos_shift(s0, c0, dth, s, c);
+      if (fabs(dth) <= 0.001953125) sincos_shift<true>(s0, c0, dth, s, c);
+      else if (fabs(dth) <= 0.06) sincos_shift<false>(s0, c0, dth, s, c);
       else sincos(x2 + dth, &s, &c);
       const Pos p1 = make_pos(g, r0 + dr, s, c);
       double Xr, Xt, Xp, Ur, Ut;
