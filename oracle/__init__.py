@@ -265,5 +265,25 @@ def pair_production(p, ptc, capacity, gamma_thr, eps_ph, p_convert, seed, step):
     return {k: v[:m].copy() for k, v in out.items()}, bool(ov.value)
 
 
+class shape_order:
+    """context manager: `with oracle.shape_order(3): ...` runs gather, deposit and rho with the cubic
+    B-spline shape ("third order spline ... through a configuration option")."""
+
+    def __init__(self, order):
+        self.order = order
+
+    def __enter__(self):
+        self.old = lib().orc_set_shape_order(C.c_int(self.order))
+        return self
+
+    def __exit__(self, *a):
+        lib().orc_set_shape_order(C.c_int(self.old))
+
+
+def shape(x):
+    lib().orc_shape.restype = C.c_double
+    return float(lib().orc_shape(C.c_double(x)))
+
+
 def num_threads():
     return lib().orc_num_threads()

@@ -20,6 +20,8 @@
 //   orc_circulation/field div B exactly preserved; div D - rho preserved; Wald/monopole
 //                         stationarity ~ Delta^2; Heun limit / order in dt
 //   orc_sort/orc_compact  = std::stable_sort / order-preserving filter (library definition)
+//   shape option 3        cubic B-spline: partition of unity, moments, C2 knots; continuity to
+//                         round-off with the spline in rho and fluxes; exact gather of linear fields
 //   orc_philox4x32_10     the published known-answer vectors (tests/golden/philox4x32_10.txt)
 //   orc_pair_production   FIDO momentum / energy conservation, eps_ph, threshold, Eq.26 fraction,
 //                         append order; recoil and split prescriptions are readings P1-P4
@@ -257,9 +259,17 @@ double fetch(const Grid& g, const double* F, const Stag& st, int i, int j) {
   return sign * F[g.idx(i, j)];
 }
 
+int g_shape_order = 1;   // shape option, see shape() below
+double shape(double x);
 double gather1(const Grid& g, const double* F, const Stag& st, double fx, double fy) {
   const double gx = fx - st.sr, gy = fy - st.sth;
   const int i0 = (int)std::floor(gx), j0 = (int)std::floor(gy);
+  if (g_shape_order == 3) {                          // sum over the 4 x 4 nodes of the spline's support
+    double acc = 0.0;
+    for (int j = j0 - 1; j <= j0 + 2; ++j)
+      for (int i = i0 - 1; i <= i0 + 2; ++i) acc += shape(gx - i) * shape(gy - j) * fetch(g, F, st, i, j);
+    return acc;
+  }
   const double wx = gx - i0, wy = gy - j0;
   return (1.0 - wy) * ((1.0 - wx) * fetch(g, F, st, i0, j0) + wx * fetch(g, F, st, i0 + 1, j0)) +
          wy * ((1.0 - wx) * fetch(g, F, st, i0, j0 + 1) + wx * fetch(g, F, st, i0 + 1, j0 + 1));
@@ -348,8 +358,21 @@ void geodesic(double a, double M, int K, const double y[6], double dt, double ep
   for (int k = 0; k < 6; ++k) yn[k] = yt[k];
 }
 
-// CIC shape function: S^(x) = max(0, 1-|x|)
-double shape(double x) { return std::max(0.0, 1.0 - std::fabs(x)); }
+// Particle shape function: first-order cloud-in-cell S^(x) = max(0, 1-|x|) "by
+// default, but a third order spline is also available ... through a configuration option": the
+// cubic B-spline  2/3 - x^2 + |x|^3/2 (|x| < 1),  (2-|x|)^3/6 (1 <= |x| < 2),  0 beyond.
+// g_shape_order is that option (1 or 3), set by orc_set_shape_order; it selects the shape used
+// by the gather, the current deposit and the charge density alike.
+int shape_ext() { return g_shape_order == 3 ? 1 : 0; }   // extra nodes of support on each side
+double shape(double x) {
+  const double ax = std::fabs(x);
+  if (g_shape_order == 3) {
+    if (ax < 1.0) return 2.0 / 3.0 - ax * ax + 0.5 * ax * ax * ax;
+    if (ax < 2.0) return (2.0 - ax) * (2.0 - ax) * (2.0 - ax) / 6.0;
+    return 0.0;
+  }
+  return std::max(0.0, 1.0 - ax);
+}
 
 // ---------------------------------------------------------------------------
 // Auxiliary fields (B9),(B11) and circulations (B8),(B10), PAPER.md:478-518,
@@ -621,8 +644,9 @@ void orc_deposit(const orc_params* p, int64_t n, const double* x1o, const double
     const double Q = ((flag[k] & 1u) ? 1.0 : -1.0) * w[k];
     const double xa = (x1o[k] - g.xi_in) / g.dxi, xb = (x1n[k] - g.xi_in) / g.dxi;
     const double ya = x2o[k] / g.dth, yb = x2dep[k] / g.dth;
-    const int ilo = (int)std::floor(std::min(xa, xb)), ihi = (int)std::floor(std::max(xa, xb)) + 1;
-    const int jlo = (int)std::floor(std::min(ya, yb)), jhi = (int)std::floor(std::max(ya, yb)) + 1;
+    const int ext = shape_ext();
+    const int ilo = (int)std::floor(std::min(xa, xb)) - ext, ihi = (int)std::floor(std::max(xa, xb)) + 1 + ext;
+    const int jlo = (int)std::floor(std::min(ya, yb)) - ext, jhi = (int)std::floor(std::max(ya, yb)) + 1 + ext;
     // (22) without /dV:  W_r,ij and W_th,ij
     for (int j = jlo; j <= jhi; ++j) {
       double acc = 0.0;  // F_r(ilo-1/2, j) = 0
@@ -750,8 +774,9 @@ void orc_rho(const orc_params* p, int64_t n, const double* x1, const double* x2,
     const double Q = ((flag[k] & 1u) ? 1.0 : -1.0) * w[k];
     const double x = (x1[k] - g.xi_in) / g.dxi, y = x2[k] / g.dth;
     const int i0 = (int)std::floor(x), j0 = (int)std::floor(y);
-    for (int j = j0; j <= j0 + 1; ++j)
-      for (int i = i0; i <= i0 + 1; ++i) rho[g.idx(i, j)] += Q * shape(x - i) * shape(y - j);
+    const int ext = shape_ext();
+    for (int j = j0 - ext; j <= j0 + 1 + ext; ++j)
+      for (int i = i0 - ext; i <= i0 + 1 + ext; ++i) rho[g.idx(i, j)] += Q * shape(x - i) * shape(y - j);
   }
   fold_rows(g, rho, false, +1.0);
   if (divide) {
@@ -953,6 +978,14 @@ int64_t orc_pair_production(const orc_params* p, int64_t n, int64_t capacity, do
     flag[k] = parent_flag;
   }
   return m;
+}
+
+double orc_shape(double x) { return shape(x); }
+// shape order option (1 = cloud-in-cell, 3 = cubic B-spline); returns the previous value
+int orc_set_shape_order(int order) {
+  const int old = g_shape_order;
+  if (order == 1 || order == 3) g_shape_order = order;
+  return old;
 }
 
 int orc_num_threads() {

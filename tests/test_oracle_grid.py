@@ -326,3 +326,80 @@ def test_sort_and_compact_definitions():
     assert np.array_equal(perm, np.argsort(key, kind="stable").astype(np.uint32))
     idx = oracle.compact(flag)
     assert np.array_equal(idx, np.nonzero((flag & 2) == 0)[0].astype(np.uint32))
+
+
+# ------------------------------------------------------------------ third-order spline shape
+def test_spline3_shape_is_the_cubic_bspline():
+    """partition of unity, first moment, variance 1/3 (cubic B-spline = 4-fold convolution of the
+    unit box: variance 4/12), support |x| < 2, C2 continuity at the knots, known values."""
+    with oracle.shape_order(3):
+        S = np.vectorize(oracle.shape)
+        assert abs(S(0.0) - 2.0 / 3.0) < 1e-16 and abs(S(1.0) - 1.0 / 6.0) < 1e-16
+        assert S(2.0) == 0.0 and S(-2.5) == 0.0 and S(1.999) > 0.0
+        nodes = np.arange(-4, 5)
+        for x in np.random.default_rng(0).uniform(-0.5, 0.5, 50):
+            wts = S(x - nodes)
+            assert abs(wts.sum() - 1.0) < 1e-15
+            assert abs((wts * nodes).sum() - x) < 1e-15
+            assert abs((wts * (nodes - x) ** 2).sum() - 1.0 / 3.0) < 1e-15
+        h = 1e-5
+        for knot in (-1.0, 0.0, 1.0):      # second derivative continuous across the knots
+            d2l = (S(knot - 2 * h) - 2 * S(knot - h) + S(knot)) / h ** 2
+            d2r = (S(knot) - 2 * S(knot + h) + S(knot + 2 * h)) / h ** 2
+            assert abs(d2l - d2r) < 1e-4
+    assert oracle.shape(0.25) == 0.75                      # option restored: cloud-in-cell
+
+
+def test_spline3_deposit_continuity_and_moments():
+    """The prefix-sum deposit (Eq.21-22) is charge conserving for any shape: with the cubic
+    B-spline in BOTH rho and the fluxes the continuity residual is round-off, incl. axis nodes."""
+    p = small_params()
+    g = oracle.Grid(p)
+    old, new, w = random_moves(p, 400, 4)
+    dt = 0.013
+    with oracle.shape_order(3):
+        F = oracle.fold_current(p, oracle.deposit(p, old, new, w, dt))
+        rho0 = oracle.rho(p, old, w, divide=False)
+        rho1 = oracle.rho(p, new, w, divide=False)
+    G = g.G
+    Fr, Fth = F[0], F[1]
+    res = (rho1 - rho0) / dt
+    div = np.zeros_like(res)
+    div[G:G + p["nth"] + 1, 1:] += Fr[G:G + p["nth"] + 1, 1:] - Fr[G:G + p["nth"] + 1, :-1]
+    div[G:G + p["nth"] + 1, :] += Fth[G:G + p["nth"] + 1, :] - Fth[G - 1:G + p["nth"], :]
+    tot = (res + div)[G:G + p["nth"] + 1, G + 2:G + p["nr"] - 1]       # support 2: nodes 2..nr-2
+    scale = np.max(np.abs(rho1)) / dt
+    assert np.max(np.abs(tot)) <= 1e-13 * scale, np.max(np.abs(tot)) / scale
+    assert np.max(np.abs(res)) > 1e-3 * scale
+    # moments (particles that stay clear of the radial edges): sum F_ph = sum Q dphi/dt
+    Q = np.where(old["flag"] & 1, 1.0, -1.0) * w
+    with oracle.shape_order(3):
+        Fraw = oracle.deposit(p, old, new, w, dt)
+    assert abs(Fraw[2].sum() - np.sum(Q * (new["x3"] - old["x3"])) / dt) < 1e-10 * np.sum(np.abs(Q)) / dt
+    # and the cubic-spline fluxes differ from the cloud-in-cell ones (the option does something)
+    F1 = oracle.deposit(p, old, new, w, dt)
+    assert np.max(np.abs(F1[0] - Fraw[0])) > 1e-3 * np.max(np.abs(F1[0]))
+
+
+def test_spline3_gather_reproduces_linear_fields():
+    """a cubic B-spline reproduces linear functions exactly: the gather of a field linear in the
+    logical coordinates returns the field at the particle (each component on its own lattice)."""
+    p = small_params(nr=24, nth=20)
+    g = oracle.Grid(p)
+    rng = np.random.default_rng(2)
+    n = 200
+    x = rng.uniform(2.0, p["nr"] - 2.0, n)
+    y = rng.uniform(2.5, p["nth"] - 2.5, n)
+    x1, x2 = p["xi_in"] + x * g.dxi, y * g.dth
+    fields, exact = [], []
+    for k, name in enumerate(inputs.FIELD_NAMES):
+        sr, sth = inputs.STAGGER[name][:2]
+        ii = np.arange(-g.G, p["nr"] + g.G + 1)[None, :] + sr
+        jj = np.arange(-g.G, p["nth"] + g.G + 1)[:, None] + sth
+        a0, a1, a2 = 0.3 + k, 0.7 - 0.1 * k, -0.2 + 0.05 * k
+        fields.append(np.ascontiguousarray(a0 + a1 * ii + a2 * jj + 0.0 * ii * jj))
+        exact.append(a0 + a1 * x + a2 * y)
+    with oracle.shape_order(3):
+        got = np.array([oracle.gather(p, fields, x1[q], x2[q]) for q in range(n)])
+    for k in range(6):
+        assert np.allclose(got[:, k], exact[k], rtol=0, atol=1e-12), k
