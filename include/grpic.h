@@ -114,6 +114,15 @@ int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes);
 int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                        grpic_current* flux, double dt, uint32_t* status, void* stream);
 
+/* The same particle step with the THIRD-ORDER (cubic B-spline) shape, the paper's configuration
+ * option ("a third order spline is also available"): gather over the 4 x 4 nodes of
+ * the spline's support on each component's own lattice, prefix-sum deposit (Eq.21-23) over the
+ * window the spline covers during the move.  In place, fluxes accumulated (+=) as in
+ * grpic_push_deposit.  The context must have been created with ng >= 3 guard nodes
+ * (GRPIC_ERR_ARG otherwise).  Parity-level implementation, not tuned. */
+int grpic_push_deposit_spline3(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
+                               grpic_current* flux, double dt, uint32_t* status, void* stream);
+
 /* Removal fused into the push (SURVEY 8(a) rows a1-a5 + a9): exactly
  * grpic_compact(in -> out) followed by grpic_push_deposit(out), in one pass over the particles.
  * `out` (must not alias `in`; in is not modified) receives, in their original order, the

@@ -336,6 +336,37 @@ def test_far_moves_take_the_general_window(G, O):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
 
 
+def test_spline3_push_deposit_parity(G, O):
+    """third-order (cubic B-spline) shape option: gather, push and deposit vs the
+    oracle run with the same option; includes axis crossers, leavers and photons."""
+    p = inputs.grid_params(48, 40, 0.99, ng=3)
+    dt = inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "wald")
+    ptc = inputs.make_particles(p, 20000, 23, "crowded", ("loguniform", 0.1, 1e3))
+    ptc["flag"] = (ptc["flag"] | np.where(np.arange(20000) % 7 == 0, 4, 0)).astype(np.uint32)
+    with O.shape_order(3):
+        ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
+    ref1, Fref1 = oracle_push_deposit(O, p, fields, ptc, dt)
+    assert np.max(np.abs(Fref[0] - Fref1[0])) > 1e-3 * np.max(np.abs(Fref1[0]))     # the option matters
+    ctx = G.Context(p, len(ptc["x1"]))
+    f_t = [ctx.to_device(f) for f in fields]
+    P = G.Particles.from_numpy(ptc)
+    F_t = ctx.zeros(3)
+    ctx.status.zero_()
+    ctx.push_deposit_spline3(P, f_t, F_t, dt)
+    torch.cuda.synchronize()
+    assert int(ctx.status.item()) == 0
+    with O.shape_order(3):
+        check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-3)
+    for c in range(3):
+        assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
+    ctx2 = G.Context(inputs.grid_params(48, 40, 0.99), 16)                         # ng = 2: refused
+    with pytest.raises(G.GrpicError):
+        ctx2.push_deposit_spline3(G.Particles.from_numpy({k: v[:16].copy() for k, v in ptc.items()}),
+                                  [ctx2.to_device(f) for f in inputs.analytic_fields(inputs.grid_params(48, 40, 0.99), "wald")],
+                                  ctx2.zeros(3), dt)
+
+
 def test_continuity_residual_gpu(G, O):
     """Charge conservation of the CUDA path itself: (rho1 - rho0) dV/dt + div F = 0 node by
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
