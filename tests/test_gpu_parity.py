@@ -2,6 +2,7 @@
 same seeded inputs.  Tolerances are BASELINE.json's: integer outputs bit-exact; x,u <= 1e-12
 relative after one step; J and fields <= 1e-11 relative; continuity residual <= 1e-13 max|rho|."""
 import math
+import os
 
 import numpy as np
 import pytest
@@ -365,6 +366,47 @@ def test_spline3_push_deposit_parity(G, O):
         ctx2.push_deposit_spline3(G.Particles.from_numpy({k: v[:16].copy() for k, v in ptc.items()}),
                                   [ctx2.to_device(f) for f in inputs.analytic_fields(inputs.grid_params(48, 40, 0.99), "wald")],
                                   ctx2.zeros(3), dt)
+
+
+def test_gpu_geodesic_orbit_invariants(G, O):
+    """Physics on the GPU path itself (Table 1 orbit (3,3,2), a = 0.995, zero
+    fields): u_phi is conserved bit for bit (U_phi = 0) and the error of the energy at infinity
+    E = alpha^2 u^0 - beta^r u_r falls as dt^2 over 120 r_g/c of the zoom-whirl orbit."""
+    vals = None
+    here = os.path.dirname(os.path.abspath(__file__))
+    for line in open(os.path.join(here, "golden", "table1_orbits.txt")):
+        if line.startswith("(3,3,2)"):
+            vals = [float(v) for v in line.split()[1:]]
+    a, _, ur, uth, uph, r0, off = vals
+    p = inputs.grid_params(32, 32, a, r_out=20.0)
+    zero = [np.zeros(inputs.grid_shape(p)) for _ in range(6)]
+    ctx = G.Context(p, 4)
+    f_t = [ctx.to_device(f) for f in zero]
+
+    def E_of(x1, x2, u1, u2, u3):
+        m = O.metric(a, 1.0, math.exp(x1), x2)
+        nrm = m["gu_rr"] * u1 ** 2 + m["gu_thth"] * u2 ** 2 + m["gu_phph"] * u3 ** 2 + 2 * m["gu_rph"] * u1 * u3
+        return m["alpha"] * math.sqrt(1.0 + nrm) - m["beta_r"] * u1
+
+    errs = []
+    for dt in (0.1, 0.05, 0.025):
+        one = dict(x1=np.array([math.log(r0)]), x2=np.array([math.pi / 2 - off]), x3=np.zeros(1),
+                   u1=np.array([ur]), u2=np.array([uth]), u3=np.array([uph]), w=np.zeros(1),
+                   flag=np.zeros(1, np.uint32))
+        one["cell"] = inputs.cells_of(p, one["x1"], one["x2"])
+        P = G.Particles.from_numpy(one)
+        F_t = ctx.zeros(3)
+        E0 = E_of(one["x1"][0], one["x2"][0], ur, uth, uph)
+        dE, n = [], int(round(120.0 / dt))
+        for s in range(n):
+            ctx.push_deposit(P, f_t, F_t, dt)
+            if s % max(1, n // 300) == 0:
+                q = P.to_numpy()
+                assert q["u3"][0] == uph and not (q["flag"][0] & 2)
+                dE.append(abs(E_of(q["x1"][0], q["x2"][0], q["u1"][0], q["u2"][0], q["u3"][0]) - E0))
+        errs.append(float(np.mean(dE)))
+    assert errs[2] < 2e-4 * abs(E0)
+    assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
 
 
 def test_continuity_residual_gpu(G, O):
