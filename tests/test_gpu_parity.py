@@ -409,6 +409,37 @@ def test_gpu_geodesic_orbit_invariants(G, O):
     assert 3.3 < errs[0] / errs[1] < 4.7 and 3.3 < errs[1] / errs[2] < 4.7, errs
 
 
+def test_gpu_field_step_preserves_divB(G, O):
+    """Invariant on the GPU path itself: the discrete div B (fluxes B^r A^B_r,
+    B^th A^B_th through the faces of every cell, areas from the library) does not change in a
+    field step, over 5 steps of random fields with the damping layer off, on a grid that spans
+    several CTA chunks and the TMA interior path."""
+    p = inputs.grid_params(200, 150, 0.95)
+    ctx = G.Context(p, 16)
+    rng = np.random.default_rng(4)
+    shape = inputs.grid_shape(p)
+    f = [rng.normal(size=shape) for _ in range(6)]
+    f_t = [ctx.to_device(x) for x in f]
+    ctx.fill_guards(f_t)
+    A = [ctx.to_host(a) for a in ctx.get_areas()]
+    Gd, nr, nth = p["ng"], p["nr"], p["nth"]
+
+    def div(ft):
+        Br, Bth = ctx.to_host(ft[3]) * A[3], ctx.to_host(ft[4]) * A[4]
+        return (Br[Gd:Gd + nth, Gd + 1:Gd + nr + 1] - Br[Gd:Gd + nth, Gd:Gd + nr]) + \
+               (Bth[Gd + 1:Gd + nth + 1, Gd:Gd + nr] - Bth[Gd:Gd + nth, Gd:Gd + nr])
+
+    d0 = div(f_t)
+    sc = np.max(np.abs(ctx.to_host(f_t[3]) * A[3]))
+    dt = inputs.courant_dt(p)
+    for _ in range(5):
+        ctx.field_step(f_t, None, dt)
+    torch.cuda.synchronize()
+    d1 = div(f_t)
+    assert np.max(np.abs(ctx.to_host(f_t[3]) - f[3][:, :])) > 1e-6        # the fields did change
+    assert np.max(np.abs(d1 - d0)) < 1e-12 * sc, np.max(np.abs(d1 - d0)) / sc
+
+
 def test_continuity_residual_gpu(G, O):
     """Charge conservation of the CUDA path itself: (rho1 - rho0) dV/dt + div F = 0 node by
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
