@@ -125,6 +125,28 @@ def boris(a, M, r, th, u, D, B, sgn, dt):
     return out
 
 
+def vay(a, M, r, th, u, D, B, sgn, dt):
+    u, D, B = (np.ascontiguousarray(v, dtype=np.float64) for v in (u, D, B))
+    out = np.zeros(3)
+    lib().orc_vay(C.c_double(a), C.c_double(M), C.c_double(r), C.c_double(th), _d(u), _d(D),
+                  _d(B), C.c_double(sgn), C.c_double(dt), _d(out))
+    return out
+
+
+class pusher:
+    """context manager: `with oracle.pusher(1): ...` makes push() use the Vay update."""
+
+    def __init__(self, which):
+        self.which = which
+
+    def __enter__(self):
+        self.old = lib().orc_set_pusher(C.c_int(self.which))
+        return self
+
+    def __exit__(self, *a):
+        lib().orc_set_pusher(C.c_int(self.old))
+
+
 def geodesic_rhs(a, M, y, eps=1.0):
     y = np.ascontiguousarray(y, dtype=np.float64)
     f = np.zeros(6)

@@ -15,6 +15,7 @@
 //   orc_areas             scipy.integrate.quad; a=0 closed forms
 //   orc_geodesic*         u_phi exact, E=-u_t ~ dt^2, Table 1 energies/periods, ISCO Omega
 //   orc_boris             norm conservation, Eq.16 residual, flat-space gyration
+//   orc_vay               E x B drift held exactly, |u| exact in pure B, agrees with Boris to O(dt^2)
 //   orc_push (+Wald)      Eq.24 energy and canonical L_phi conservation
 //   orc_deposit           discrete continuity Eq.21 to round-off; whole-row brute force
 //   orc_circulation/field div B exactly preserved; div D - rho preserved; Wald/monopole
@@ -325,6 +326,52 @@ void boris(const Metric& m, const double u[3], const double D[3], const double B
   for (int k = 0; k < 3; ++k) uout[k] = up[k] + sgn * (m.alpha * dt / 2.0) * Dlo[k];  // (17)
 }
 
+// Vay pusher in the FIDO frame ("a transformation to the FIDO frame and ... the
+// Vay momentum update there (Vay 2008)").  Readings V1-V3: orthonormal triad
+//   e_(1) = sqrt(gamma^rr) (d_r - (gamma_rphi/gamma_phiphi) d_phi),  e_(2) = d_theta/sqrt(gamma_thth),
+//   e_(3) = d_phi/sqrt(gamma_phiphi)   (right-handed: sqrt(gamma) eps_ijk e1^i e2^j e3^k = 1);
+// FIDO proper time of the step alpha*dt; D^i, B^i are the fields the FIDO measures.  Vay (2008):
+//   u' = u + h (E + v x B / 2),  v = u/Gamma,  h = (q/m) alpha dt,  tau = (h/2) B,  u* = u'.tau,
+//   sigma = 1 + u'^2 - tau^2,  Gamma1^2 = (sigma + sqrt(sigma^2 + 4 (tau^2 + u*^2)))/2,
+//   t = tau/Gamma1,  u1 = (u' + (u'.t) t + u' x t)/(1 + t^2).
+void vay(const Metric& m, const double u[3], const double D[3], const double B[3], double sgn, double dt,
+         double uout[3]) {
+  const double sgrr = std::sqrt(m.gu_rr), sth = std::sqrt(m.g_thth), sph = std::sqrt(m.g_phph);
+  const double k = m.g_rph / m.g_phph;
+  auto vec_hat = [&](const double V[3], double out[3]) {          // contravariant -> orthonormal
+    out[0] = V[0] / sgrr;
+    out[1] = sth * V[1];
+    out[2] = (m.g_rph * V[0] + m.g_phph * V[2]) / sph;
+  };
+  const double uh[3] = {sgrr * (u[0] - k * u[2]), u[1] / sth, u[2] / sph};   // covariant -> orthonormal
+  double E[3], Bh[3];
+  vec_hat(D, E);
+  vec_hat(B, Bh);
+  const double h = sgn * m.alpha * dt;
+  const double G0 = std::sqrt(1.0 + uh[0] * uh[0] + uh[1] * uh[1] + uh[2] * uh[2]);
+  const double v[3] = {uh[0] / G0, uh[1] / G0, uh[2] / G0};
+  double up[3];
+  up[0] = uh[0] + h * (E[0] + 0.5 * (v[1] * Bh[2] - v[2] * Bh[1]));
+  up[1] = uh[1] + h * (E[1] + 0.5 * (v[2] * Bh[0] - v[0] * Bh[2]));
+  up[2] = uh[2] + h * (E[2] + 0.5 * (v[0] * Bh[1] - v[1] * Bh[0]));
+  const double tau[3] = {0.5 * h * Bh[0], 0.5 * h * Bh[1], 0.5 * h * Bh[2]};
+  const double tau2 = tau[0] * tau[0] + tau[1] * tau[1] + tau[2] * tau[2];
+  const double ustar = up[0] * tau[0] + up[1] * tau[1] + up[2] * tau[2];
+  const double sigma = 1.0 + up[0] * up[0] + up[1] * up[1] + up[2] * up[2] - tau2;
+  const double G1 = std::sqrt(0.5 * (sigma + std::sqrt(sigma * sigma + 4.0 * (tau2 + ustar * ustar))));
+  const double t[3] = {tau[0] / G1, tau[1] / G1, tau[2] / G1};
+  const double t2 = t[0] * t[0] + t[1] * t[1] + t[2] * t[2];
+  const double udt = up[0] * t[0] + up[1] * t[1] + up[2] * t[2];
+  const double sc = 1.0 / (1.0 + t2);
+  const double u1[3] = {sc * (up[0] + udt * t[0] + (up[1] * t[2] - up[2] * t[1])),
+                        sc * (up[1] + udt * t[1] + (up[2] * t[0] - up[0] * t[2])),
+                        sc * (up[2] + udt * t[2] + (up[0] * t[1] - up[1] * t[0]))};
+  uout[0] = u1[0] / sgrr + u1[2] * m.g_rph / sph;                 // orthonormal -> covariant
+  uout[1] = sth * u1[1];
+  uout[2] = sph * u1[2];
+}
+int g_pusher = 0;   // momentum update of orc_push: 0 = generalised Boris (default), 1 = Vay in the FIDO frame
+
 // ---------------------------------------------------------------------------
 // Geodesic right-hand sides X^i, U_i of Eq.(12) without F_i,
 // y = (r, theta, phi, u_r, u_theta, u_phi); eps = 1 massive, 0 photon (:153).
@@ -544,6 +591,16 @@ void orc_boris(double a, double M, double r, double th, const double* u, const d
                const double* B, double sgn, double dt, double* uout) {
   boris(metric(a, M, r, th), u, D, B, sgn, dt, uout);
 }
+void orc_vay(double a, double M, double r, double th, const double* u, const double* D,
+             const double* B, double sgn, double dt, double* uout) {
+  vay(metric(a, M, r, th), u, D, B, sgn, dt, uout);
+}
+// momentum update used by orc_push (0 = Boris, 1 = Vay); returns the previous value
+int orc_set_pusher(int which) {
+  const int old = g_pusher;
+  if (which == 0 || which == 1) g_pusher = which;
+  return old;
+}
 
 void orc_geodesic_rhs(double a, double M, const double* y, double eps, double* f) {
   geodesic_rhs(a, M, y, eps, f);
@@ -601,7 +658,8 @@ void orc_push(const orc_params* p, const double* Dr, const double* Dth, const do
       B[0] = gather1(g, Br, ST_Br, fx, fy);
       B[1] = gather1(g, Bth, ST_Bth, fx, fy);
       B[2] = gather1(g, Bph, ST_Bph, fx, fy);
-      boris(metric(g.a, g.M, r, th), u, D, B, sgn, dt, ub);
+      if (g_pusher == 1) vay(metric(g.a, g.M, r, th), u, D, B, sgn, dt, ub);
+      else boris(metric(g.a, g.M, r, th), u, D, B, sgn, dt, ub);
     }
     const double y[6] = {r, th, x3[k], ub[0], ub[1], ub[2]};
     double yn[6];

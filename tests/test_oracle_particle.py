@@ -434,3 +434,84 @@ def test_pair_production_conserves_fido_momentum_and_energy():
     assert ov2 and len(out2["x1"]) == n + 5
     for k in out2:
         assert np.array_equal(out2[k][n:], out[k][n:n + 5]), k
+
+
+# ------------------------------------------------------------------ Vay pusher in the FIDO frame
+def _triad_up(m, Vhat):
+    """orthonormal FIDO components -> contravariant V^i (inverse of the oracle's own map, written
+    from the triad e_(1) = sqrt(g^rr)(d_r - g_rph/g_phph d_ph), e_(2) = d_th/sqrt(g_thth), e_(3) = d_ph/sqrt(g_phph))."""
+    sgrr, sth, sph = math.sqrt(m["gu_rr"]), math.sqrt(m["g_thth"]), math.sqrt(m["g_phph"])
+    k = m["g_rph"] / m["g_phph"]
+    return np.array([sgrr * Vhat[0], Vhat[1] / sth, -sgrr * k * Vhat[0] + Vhat[2] / sph])
+
+
+def _hat_of_cov(m, u):
+    sgrr, sth, sph = math.sqrt(m["gu_rr"]), math.sqrt(m["g_thth"]), math.sqrt(m["g_phph"])
+    return np.array([sgrr * (u[0] - m["g_rph"] / m["g_phph"] * u[2]), u[1] / sth, u[2] / sph])
+
+
+def _cov_of_hat(m, uh):
+    sgrr, sth, sph = math.sqrt(m["gu_rr"]), math.sqrt(m["g_thth"]), math.sqrt(m["g_phph"])
+    return np.array([uh[0] / sgrr + uh[2] * m["g_rph"] / sph, sth * uh[1], sph * uh[2]])
+
+
+def test_vay_holds_the_ExB_drift_exactly_and_boris_does_not():
+    """Vay (2008): a particle moving with the E x B drift velocity feels no net force and must stay
+    at that velocity for ANY time step; the Boris update only does to O(dt^2).  Fields and momentum
+    are set up in the orthonormal FIDO frame at a point of the a = 0.9 Kerr metric."""
+    a, M, r, th = 0.9, 1.0, 3.0, 1.0
+    m = oracle.metric(a, M, r, th)
+    assert abs(m["sqrtg"] * math.sqrt(m["gu_rr"]) / (math.sqrt(m["g_thth"]) * math.sqrt(m["g_phph"])) - 1.0) < 1e-13
+    Ehat, Bhat = np.array([0.0, 0.6, 0.0]), np.array([0.0, 0.0, 1.0])
+    vd = np.cross(Ehat, Bhat) / Bhat.dot(Bhat)                        # (0.6, 0, 0)
+    G = 1.0 / math.sqrt(1.0 - vd.dot(vd))
+    uh0 = G * vd
+    D, B = _triad_up(m, Ehat), _triad_up(m, Bhat)
+    u0 = _cov_of_hat(m, uh0)
+    for dt in (0.01, 1.0, 30.0):
+        u = u0.copy()
+        for _ in range(50):
+            u = oracle.vay(a, M, r, th, u, D, B, +1.0, dt)
+        assert np.max(np.abs(_hat_of_cov(m, u) - uh0)) < 1e-12, dt
+    ub = oracle.boris(a, M, r, th, u0, D, B, +1.0, 1.0)
+    assert np.max(np.abs(_hat_of_cov(m, ub) - uh0)) > 1e-3            # Boris leaves the drift at large dt
+
+
+def test_vay_pure_B_conserves_energy_and_matches_boris_to_second_order():
+    a, M, r, th = 0.7, 1.0, 2.5, 0.8
+    m = oracle.metric(a, M, r, th)
+    rng = np.random.default_rng(3)
+    u = rng.normal(size=3) * np.array([1.0, 2.0, 2.0])
+    B = rng.normal(size=3)
+    nrm = lambda w: (m["gu_rr"] * w[0] ** 2 + m["gu_thth"] * w[1] ** 2 + m["gu_phph"] * w[2] ** 2
+                     + 2 * m["gu_rph"] * w[0] * w[2])
+    v = u.copy()
+    for _ in range(100):
+        v = oracle.vay(a, M, r, th, v, np.zeros(3), B, -1.0, 0.3)
+    assert abs(nrm(v) / nrm(u) - 1.0) < 1e-13                          # |u| exact in a pure magnetic field
+    # with E != 0 the two pushers are both second order: their difference falls as dt^3 per step
+    D = rng.normal(size=3) * 0.3
+    d = []
+    for dt in (0.04, 0.02, 0.01):
+        d.append(np.max(np.abs(oracle.vay(a, M, r, th, u, D, B, 1.0, dt) - oracle.boris(a, M, r, th, u, D, B, 1.0, dt))))
+    assert 6.0 < d[0] / d[1] < 10.0 and 6.0 < d[1] / d[2] < 10.0, d
+
+
+def test_push_with_vay_option_uses_vay():
+    from paper_2503_04558_b200 import inputs
+    p = inputs.grid_params(24, 20, 0.9)
+    fields = inputs.analytic_fields(p, "wald")
+    ptc = inputs.make_particles(p, 50, 3, "logical", ("loguniform", 0.1, 10.0))
+    dt = inputs.courant_dt(p)
+    with oracle.pusher(1):
+        nv = oracle.push(p, fields, ptc, dt)
+    nb = oracle.push(p, fields, ptc, dt)
+    assert np.max(np.abs(nv["u1"] - nb["u1"])) > 0 and np.allclose(nv["u1"], nb["u1"], rtol=1e-3, atol=1e-6)
+    # one particle by hand: gather -> vay -> geodesic
+    k = 7
+    D6 = oracle.gather(p, fields, ptc["x1"][k], ptc["x2"][k])
+    sgn = 1.0 if ptc["flag"][k] & 1 else -1.0
+    r, th = math.exp(ptc["x1"][k]), ptc["x2"][k]
+    ub = oracle.vay(p["a"], p["M"], r, th, [ptc["u1"][k], ptc["u2"][k], ptc["u3"][k]], D6[:3], D6[3:], sgn, dt)
+    yn = oracle.geodesic(p["a"], p["M"], 3, np.array([r, th, ptc["x3"][k], *ub]), dt)
+    assert abs(math.log(yn[0]) - nv["x1"][k]) < 1e-15 and abs(yn[3] - nv["u1"][k]) < 1e-15
