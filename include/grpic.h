@@ -123,6 +123,17 @@ int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields*
 int grpic_push_deposit_spline3(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                                grpic_current* flux, double dt, uint32_t* status, void* stream);
 
+/* The particle step with the paper's method variants selected by argument (same in-place
+ * semantics as grpic_push_deposit; general, untuned kernel):
+ *   shape_order = 1 (cloud-in-cell) or 3 (cubic B-spline, needs ng >= 3);
+ *   pusher = 0: generalised Boris (Eq.16-19); 1: Vay update in the FIDO frame (Vay
+ *   2008) with the triad e_(1) = sqrt(gamma^rr)(d_r - gamma_rphi/gamma_phiphi d_phi),
+ *   e_(2) = d_theta/sqrt(gamma_thth), e_(3) = d_phi/sqrt(gamma_phiphi) and proper time alpha*dt.
+ * grpic_push_deposit_spline3 is (3, 0).  Other values: GRPIC_ERR_ARG. */
+int grpic_push_deposit_variant(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
+                               grpic_current* flux, double dt, int32_t shape_order, int32_t pusher,
+                               uint32_t* status, void* stream);
+
 /* Removal fused into the push (SURVEY 8(a) rows a1-a5 + a9): exactly
  * grpic_compact(in -> out) followed by grpic_push_deposit(out), in one pass over the particles.
  * `out` (must not alias `in`; in is not modified) receives, in their original order, the

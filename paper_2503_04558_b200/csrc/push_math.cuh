@@ -131,6 +131,41 @@ __device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double alp
   ur = fma(k, Dr, pr); ut = fma(k, Dt, pt); up = fma(k, Dp, pp);
 }
 
+// Vay pusher in the FIDO frame (Vay 2008), full dt.  Orthonormal triad
+// e_(1) = sqrt(gamma^rr)(d_r - gamma_rphi/gamma_phiphi d_phi), e_(2) = d_theta/sqrt(gamma_thth),
+// e_(3) = d_phi/sqrt(gamma_phiphi); FIDO proper time alpha*dt.  D, B contravariant, u covariant.
+__device__ __forceinline__ void vay(const GridDev& g, const Pos& p, double alpha, double sgn, double dt,
+                                    const double D[3], const double B[3], double& ur, double& ut, double& up) {
+  const double s2 = p.s * p.s;
+  const double g_rp = -g.a * s2 * p.zp1, g_pp = s2 * fma(g.a2 * s2, p.zp1, p.rho2);
+  const double gu_rr = fma(p.r2a2, p.R, -p.beta);
+  const double sgrr = sqrt(gu_rr), sth = sqrt(p.rho2), sph = sqrt(g_pp);
+  const double k = g_rp / g_pp;
+  const double uh0 = sgrr * (ur - k * up), uh1 = ut / sth, uh2 = up / sph;
+  const double E0 = D[0] / sgrr, E1 = sth * D[1], E2 = (g_rp * D[0] + g_pp * D[2]) / sph;
+  const double B0 = B[0] / sgrr, B1 = sth * B[1], B2 = (g_rp * B[0] + g_pp * B[2]) / sph;
+  const double h = sgn * alpha * dt;
+  const double iG0 = 1.0 / sqrt(1.0 + uh0 * uh0 + uh1 * uh1 + uh2 * uh2);
+  const double v0 = uh0 * iG0, v1 = uh1 * iG0, v2 = uh2 * iG0;
+  const double p0 = uh0 + h * (E0 + 0.5 * (v1 * B2 - v2 * B1));
+  const double p1 = uh1 + h * (E1 + 0.5 * (v2 * B0 - v0 * B2));
+  const double p2 = uh2 + h * (E2 + 0.5 * (v0 * B1 - v1 * B0));
+  const double t0 = 0.5 * h * B0, t1 = 0.5 * h * B1, t2 = 0.5 * h * B2;
+  const double tau2 = t0 * t0 + t1 * t1 + t2 * t2;
+  const double ustar = p0 * t0 + p1 * t1 + p2 * t2;
+  const double sigma = 1.0 + p0 * p0 + p1 * p1 + p2 * p2 - tau2;
+  const double G1 = sqrt(0.5 * (sigma + sqrt(sigma * sigma + 4.0 * (tau2 + ustar * ustar))));
+  const double w0 = t0 / G1, w1 = t1 / G1, w2 = t2 / G1;
+  const double udt = p0 * w0 + p1 * w1 + p2 * w2;
+  const double sc = 1.0 / (1.0 + w0 * w0 + w1 * w1 + w2 * w2);
+  const double n0 = sc * (p0 + udt * w0 + (p1 * w2 - p2 * w1));
+  const double n1 = sc * (p1 + udt * w1 + (p2 * w0 - p0 * w2));
+  const double n2 = sc * (p2 + udt * w2 + (p0 * w1 - p1 * w0));
+  ur = n0 / sgrr + n2 * g_rp / sph;
+  ut = sth * n1;
+  up = sph * n2;
+}
+
 // F[...] += v unless v == 0: one DSETP + one predicated RED.E.ADD.F64 (no divergent branch, so
 // no BSSY/BSYNC pair around every one of the 40 window slots).
 __device__ __forceinline__ void red_add(double* p, double v) {

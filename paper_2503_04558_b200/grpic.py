@@ -47,7 +47,7 @@ class CurrentC(C.Structure):
 
 EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_areas",
            "grpic_workspace_bytes", "grpic_set_workspace", "grpic_push_deposit",
-           "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3",
+           "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_sort", "grpic_compact", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
@@ -224,6 +224,12 @@ class Context:
         ps, fs, js = ptc.struct(), self._fields(fields), self._current(flux)
         _check(load().grpic_push_deposit_spline3(self.h, C.byref(ps), C.byref(fs), C.byref(js),
                                                  C.c_double(dt), _ptr(self.status, _up), _stream()))
+
+    def push_deposit_variant(self, ptc, fields, flux, dt, shape_order=1, pusher=0):
+        ps, fs, js = ptc.struct(), self._fields(fields), self._current(flux)
+        _check(load().grpic_push_deposit_variant(self.h, C.byref(ps), C.byref(fs), C.byref(js), C.c_double(dt),
+                                                 C.c_int32(shape_order), C.c_int32(pusher),
+                                                 _ptr(self.status, _up), _stream()))
 
     def push_deposit_compact(self, src, dst, fields, flux, dt, n_alive):
         """compact(src -> dst) fused with push_deposit(dst); n_alive: int64 device tensor (1)."""

@@ -491,6 +491,34 @@ def test_gpu_coupled_loop_preserves_gauss_law(G, O):
     assert np.max(np.abs((g1 - g0)[sel])) < 1e-11 * sc, np.max(np.abs((g1 - g0)[sel])) / sc
 
 
+@pytest.mark.parametrize("order,pusher", [(1, 0), (1, 1), (3, 1)])
+def test_push_deposit_variants_parity(G, O, order, pusher):
+    """grpic_push_deposit_variant vs the oracle with the same options: shape order 1 / 3
+     and pusher Boris / Vay in the FIDO frame.  (1, 0) must also
+    agree with the tuned default kernel's result through the oracle."""
+    p = inputs.grid_params(48, 40, 0.99, ng=3)
+    dt = inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "wald")
+    ptc = inputs.make_particles(p, 20000, 41, "crowded", ("loguniform", 0.1, 1e3))
+    with O.shape_order(order), O.pusher(pusher):
+        ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
+    ctx = G.Context(p, len(ptc["x1"]))
+    f_t = [ctx.to_device(f) for f in fields]
+    P = G.Particles.from_numpy(ptc)
+    F_t = ctx.zeros(3)
+    ctx.status.zero_()
+    ctx.push_deposit_variant(P, f_t, F_t, dt, shape_order=order, pusher=pusher)
+    torch.cuda.synchronize()
+    assert int(ctx.status.item()) == 0
+    with O.shape_order(order), O.pusher(pusher):
+        check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-3)
+    for c in range(3):
+        assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
+    if pusher == 1:     # the option matters: Vay and Boris momenta differ at O(dt^3) per step
+        refb = O.push(p, fields, ptc, dt)
+        assert np.max(np.abs(refb["u1"] - ref["u1"])) > 0
+
+
 def test_continuity_residual_gpu(G, O):
     """Charge conservation of the CUDA path itself: (rho1 - rho0) dV/dt + div F = 0 node by
     node to <= 1e-13 max|rho dV|/dt, using the library's own rho deposit."""
