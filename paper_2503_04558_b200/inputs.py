@@ -109,11 +109,29 @@ def _monopole(a, M, B0, r, th):
     return Br, Bth, Bph, Er, Eth, np.zeros_like(Er)
 
 
+def _wald_nonrotating(a, M, B0, r, th):
+    """Eq.(25), PAPER.md:315-317 (reading G6): the a = 0 Wald potential A_phi = (B0/2) gamma_phiphi
+    placed in the spinning metric: B^r = d_theta A_phi / sqrt(gamma), B^theta = -d_r A_phi / sqrt(gamma),
+    B^phi = 0, E_i = 0 (initial state of the vacuum relaxation test, Section 3.2)."""
+    s, c = np.sin(th), np.cos(th)
+    rho2 = r * r + a * a * c * c
+    F = rho2 + a * a * s * s + 2.0 * M * r * a * a * s * s / rho2          # gamma_phiphi = s^2 F
+    dFr = 2.0 * r + 2.0 * M * a * a * s * s * (rho2 - 2.0 * r * r) / rho2 ** 2
+    dFt = 4.0 * M * r * a * a * s * c * (r * r + a * a) / rho2 ** 2
+    sg = kerr_schild(a, M, r, th)["sqrtg"]
+    with np.errstate(divide="ignore", invalid="ignore"):
+        Br = 0.5 * B0 * (2.0 * s * c * F + s * s * dFt) / sg
+        Bth = -0.5 * B0 * s * s * dFr / sg
+    z = np.zeros_like(Br)
+    return Br, Bth, z, z, z, z
+
+
 def analytic_DB(a, M, B0, r, th, kind):
     """Contravariant D^i, B^i at points (r, th) from the analytic E_i, B^i through Eq.(6)
     (PAPER.md:84): alpha D_i = E_i - e_ijk beta^j B^k, D^i = gamma^ij D_j."""
     r, th = np.broadcast_arrays(np.asarray(r, dtype=np.float64), np.asarray(th, dtype=np.float64))
-    Br, Bth, Bph, Er, Eth, Eph = (_wald if kind == "wald" else _monopole)(a, M, B0, r, th)
+    fn = {"wald": _wald, "monopole": _monopole, "wald0": _wald_nonrotating}[kind]
+    Br, Bth, Bph, Er, Eth, Eph = fn(a, M, B0, r, th)
     m = kerr_schild(a, M, r, th)
     e_r = Er
     e_th = Eth + m["sqrtg"] * m["beta_r"] * Bph
