@@ -217,13 +217,15 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   }
   const uint32_t flag = T.flag[tid];
   const bool active = !(flag & 2u);
-  uint32_t kd = k;                                   // where this particle's result is stored
   if (COMPACT) {
+    // where this particle's result goes: offsets[tile32] + rank among the live lanes.  Both are
+    // parked in the tile's own shared-memory slots (the flag word's upper bits, the weight slot of
+    // a dead lane is not needed) instead of registers that would live across the whole push.
     const uint32_t live = __ballot_sync(0xffffffffu, active);
     const uint32_t obase = obase_next;
     if (tile32 + tstride * kWarps < ntiles32) obase_next = offsets[tile32 + tstride * kWarps];
     if (tile32 == ntiles32 - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
-    kd = obase + __popc(live & ((1u << lane) - 1u));
+    T.flag[tid] = flag | ((obase + __popc(live & ((1u << lane) - 1u))) << 3);   // kd < 2^29
   }
 
   if (active) {
@@ -359,6 +361,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
     }
+    const uint32_t kd = COMPACT ? (T.flag[tid] >> 3) : k;
     __stcs(dst.x1 + kd, x1n); __stcs(dst.x2 + kd, th); __stcs(dst.x3 + kd, ph);   // streaming stores
     __stcs(dst.u1 + kd, vr); __stcs(dst.u2 + kd, vt); __stcs(dst.u3 + kd, up);
     if (COMPACT) __stcs(dst.w + kd, T.w[tid]);
