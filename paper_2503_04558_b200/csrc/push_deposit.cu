@@ -25,7 +25,19 @@
 
 namespace {
 
-constexpr int kBlock = 128;
+// CTA size and the two occupancy settings (resident CTAs per SM) the launcher chooses between.
+// Measured at 1e8 particles, compacting / in place (ms): 256 threads x 2: 6.87 / 6.53; 128 x 4: 6.70 / 6.36,
+// 128 x 5: 7.11 / 6.22; 64 x 8: 6.62 / 6.27, 64 x 10: 6.99 / 6.11; 32 x 16: 7.00 / 6.56.
+#ifndef GRPIC_PD_BLOCK
+#define GRPIC_PD_BLOCK 64
+#endif
+#ifndef GRPIC_PD_MA
+#define GRPIC_PD_MA 8      // 126 registers per thread: the compacting variant
+#endif
+#ifndef GRPIC_PD_MB
+#define GRPIC_PD_MB 10     // 96 registers per thread: the in-place variant
+#endif
+constexpr int kBlock = GRPIC_PD_BLOCK;
 
 // Charge-conserving deposit of one move (Eq.21-23) on the 3x3-node window anchored at the
 // lower of the old and new cell in each direction: a move of less than one cell touches at
@@ -135,14 +147,14 @@ struct __align__(128) PtcTile {
 };
 constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
 
-// Persistent kernel.  A CTA walks the 128-particle tiles blockIdx.x, + gridDim.x, ...; a ring of
+// Persistent kernel.  A CTA walks the kBlock-particle tiles blockIdx.x, + gridDim.x, ...; a ring of
 // shared-memory stages holds the particle state of the current and the next tiles, each filled by
 // eight 1-D bulk TMA copies (block-uniform addresses: no per-warp address arithmetic).  There is
-// no block-wide barrier in the loop: the four warps run independently, each waits on the
+// no block-wide barrier in the loop: the warps run independently, each waits on the
 // stage's mbarrier for its data, counts itself out of the stage when it has read it, and the
 // last warp out refills the stage with the tile kPdStages steps ahead.  A warp that takes a slow path
 // (far deposit, large-angle sincos) delays the others by at most one tile.  The last, partial
-// tile (n % 128 != 0) is staged with plain loads.
+// tile (n % kBlock != 0) is staged with plain loads.
 //
 // COMPACT: the results are stored to `dst` at offsets[tile] + rank among the tile's live lanes
 // (offsets = exclusive scan of the per-tile live counts of `ptc`), i.e. particles already
@@ -415,15 +427,15 @@ template <bool COMPACT>
 int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
                           const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
                           const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
-  // tuning knob (read once): resident CTAs per SM.  Measured at 1e8 particles: in place 6.65 ms
-  // (5 CTAs, 96 registers) vs 6.78 ms (4 CTAs); compacting 7.50 ms vs 7.16 ms
+  // tuning knob (read once): GRPIC_PD_MINB=4 selects the 126-register build (GRPIC_PD_MA CTAs per
+  // SM), anything else the 96-register one (GRPIC_PD_MB); defaults: compacting -> 126, in place -> 96
   static int minb = -1;
   if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : (COMPACT ? 4 : 5); }
   if (ctx->p.geo_iters != 3)
-    return launch_push_deposit<4, COMPACT, 0>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 0>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
   if (minb == 4)
-    return launch_push_deposit<4, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
-  return launch_push_deposit<5, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+  return launch_push_deposit<GRPIC_PD_MB, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
 }
 
 // live particles per 32-particle tile: each thread reads four flags (16 bytes), eight threads
