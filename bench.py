@@ -40,15 +40,15 @@ UNIT = "particle-steps/s"
 # arithmetic"): FP64 pipe instructions of the method as stated (S4/S5 of SURVEY 8(c)) and
 # compulsory HBM bytes (particle state in + out; grid traffic amortised when sorted).
 # FP64: the warp-level FP64-pipe instructions (DFMA/DMUL/DADD/DSETP) the kernel EXECUTES per
-# particle, counted on ncu's source page (profiles/r01g): 623 (689 at r01c, 647 at r01f).
+# particle, counted on ncu's source page (profiles/r01i): 623 (689 at r01c, 647 at r01f).
 # An operation count of the method as the paper states it is higher (~1190-1350); the
 # executed count is used so that `frac` equals the FP64 pipe utilisation ncu reports and is never
 # flattered by it.
 FP64_INSTR_PER_PARTICLE = 623.0
 HBM_BYTES_PER_PARTICLE = 119.0
 # dram__bytes_read.sum + dram__bytes_write.sum of push_deposit_kernel<.,COMPACT> per live particle,
-# from the one `ncu --set full` capture of profiles/r01g (6.58 GB + 6.55 GB for 99.8e6 particles)
-NCU_DRAM_BYTES_PER_PARTICLE = 131.6
+# from the one `ncu --set full` capture of profiles/r01i (6.79 GB + 6.70 GB for 99.8e6 particles)
+NCU_DRAM_BYTES_PER_PARTICLE = 135.2
 # nominal FP64 pipe: 148 SMs x 64 DFMA lanes/clk x 1.965 GHz (B200)
 FP64_NOMINAL_INSTR_PER_S = 148 * 64 * 1.965e9
 
@@ -301,7 +301,7 @@ def run_ours(args):
         "achieved": 2.0 * fp64_ach / 1e12, "peak": 2.0 * fp64_peak_sust / 1e12, "unit": "TFLOP/s",
         "frac": max(t_alu, t_hbm) / (pd_ms * 1e-3),
         "traffic": NCU_DRAM_BYTES_PER_PARTICLE * per_launch,
-        "traffic_source": "ncu --set full capture of profiles/r01g (bytes per particle) x particles per launch",
+        "traffic_source": "ncu --set full capture of profiles/r01i (bytes per particle) x particles per launch",
         "peak_source": "FP64 DFMA chain measured live on this device after the timed loop "
                        "(sustained clocks); 2 flop per FP64 pipe instruction",
         "peak_burst": 2.0 * fp64_peak_burst / 1e12,
