@@ -22,7 +22,7 @@ namespace {
 
 constexpr int kOutCols = 28;   // output columns per warp
 #ifndef GRPIC_FS_WARPS
-#define GRPIC_FS_WARPS 4
+#define GRPIC_FS_WARPS 2
 #endif
 #ifndef GRPIC_FS_STAGES
 #define GRPIC_FS_STAGES 2
@@ -126,7 +126,8 @@ __device__ __forceinline__ double shfl_dn1(double v) { return __shfl_down_sync(0
 // 32 doubles, each fetched by ONE 256-byte bulk TMA copy issued by lanes 0..17 in parallel and
 // signalled on the stage's mbarrier.  Packet jj+kStages is requested as soon as packet jj is
 // consumed, so kStages rows are always in flight per warp without holding a register or an L1
-// line (measured: 2 stages x 4 warps per CTA is best; deeper rings cost occupancy).
+// line (measured, field step at 2048^2 / 4096^2: 2 warps x 2 stages per CTA 1.58 / 5.39 ms, 4 x 2
+// 1.63 / 5.49, 2 x 3 1.62 / 5.56; deeper rings cost occupancy).
 constexpr int kSeg = 18;
 template <int MODE, bool FAST, bool TMA>
 __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A, int lane, int ibase,
