@@ -71,6 +71,7 @@ def parse():
     ap.add_argument("--grid", type=int, default=0, help="override nr = nth")
     ap.add_argument("--sort-every", type=int, default=-1)
     ap.add_argument("--e2e-steps", type=int, default=3)
+    ap.add_argument("--e2e-chunk", type=int, default=0, help="particles per chunk of grpic_step_host (0 = library default)")
     ap.add_argument("--separate-compact", action="store_true",
                     help="run compaction as its own pass instead of fused into the push")
     ap.add_argument("--no-e2e", action="store_true")
@@ -450,7 +451,7 @@ def run_e2e(args, ctx, grpic, state, fields0, flux, dt, filt, bg, world, dist):
     host["n"] = n
     hJ = [torch.empty(f.shape, dtype=f.dtype).pin_memory() for f in flux]
     fields = [f.clone() for f in fields0]
-    ctx.step_host(host, fields, dt, host_J=hJ, background=bg, filter_passes=filt)     # warm-up, allocates staging
+    ctx.step_host(host, fields, dt, host_J=hJ, background=bg, filter_passes=filt, chunk=args.e2e_chunk)   # warm-up, allocates staging
     torch.cuda.synchronize()
     units, h2d, d2h = 0, 0, 0
     jbytes = sum(j.numel() * j.element_size() for j in hJ)
@@ -459,7 +460,7 @@ def run_e2e(args, ctx, grpic, state, fields0, flux, dt, filt, bg, world, dist):
     e0.record()
     for _ in range(KE):
         n_in = host["n"]
-        n_out = ctx.step_host(host, fields, dt, host_J=hJ, background=bg, filter_passes=filt)
+        n_out = ctx.step_host(host, fields, dt, host_J=hJ, background=bg, filter_passes=filt, chunk=args.e2e_chunk)
         units += n_in
         h2d += 60 * n_in
         d2h += 64 * n_out + jbytes + 4
