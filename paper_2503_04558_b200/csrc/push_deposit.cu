@@ -144,6 +144,7 @@ constexpr int kPdStages = GRPIC_PD_STAGES;   // particle tiles in flight per CTA
 struct __align__(128) PtcTile {
   double x1[kBlock], x2[kBlock], x3[kBlock], u1[kBlock], u2[kBlock], u3[kBlock], w[kBlock];
   uint32_t flag[kBlock];
+  uint32_t dest[kBlock];   // COMPACT: output index of each particle (written by its own thread, not by TMA)
 };
 constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
 
@@ -230,14 +231,13 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   const uint32_t flag = T.flag[tid];
   const bool active = !(flag & 2u);
   if (COMPACT) {
-    // where this particle's result goes: offsets[tile32] + rank among the live lanes.  Both are
-    // parked in the tile's own shared-memory slots (the flag word's upper bits, the weight slot of
-    // a dead lane is not needed) instead of registers that would live across the whole push.
+    // where this particle's result goes: offsets[tile32] + rank among the live lanes, parked in
+    // the tile's shared memory instead of a register that would live across the whole push
     const uint32_t live = __ballot_sync(0xffffffffu, active);
     const uint32_t obase = obase_next;
     if (tile32 + tstride * kWarps < ntiles32) obase_next = offsets[tile32 + tstride * kWarps];
     if (tile32 == ntiles32 - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
-    T.flag[tid] = flag | ((obase + __popc(live & ((1u << lane) - 1u))) << 3);   // kd < 2^29
+    T.dest[tid] = obase + __popc(live & ((1u << lane) - 1u));
   }
 
   if (active) {
@@ -373,7 +373,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
     }
-    const uint32_t kd = COMPACT ? (T.flag[tid] >> 3) : k;
+    const uint32_t kd = COMPACT ? T.dest[tid] : k;
     __stcs(dst.x1 + kd, x1n); __stcs(dst.x2 + kd, th); __stcs(dst.x3 + kd, ph);   // streaming stores
     __stcs(dst.u1 + kd, vr); __stcs(dst.u2 + kd, vt); __stcs(dst.u3 + kd, up);
     if (COMPACT) __stcs(dst.w + kd, T.w[tid]);
