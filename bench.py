@@ -311,6 +311,9 @@ def run_ours(args):
         "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
                 "bytes_per_particle": HBM_BYTES_PER_PARTICLE, "peak_source": hbm_src},
         "launch_ms": pd_ms, "particles_per_launch": per_launch,
+        # grpic_measure_fp64_issue: cycles per warp FP64 instruction per scheduler
+        "issue_model_cycles": dict(zip(("dfma_2reg", "dfma_3reg", "dmul", "dmul_plus_3_int"),
+                                       ctx.measure_fp64_issue())),
     }
     # field step: cell-updates/s and HBM fraction (192 B per cell-sweep, N+1 sweeps)
     kernels = {}
