@@ -49,6 +49,9 @@ HBM_BYTES_PER_PARTICLE = 119.0
 # dram__bytes_read.sum + dram__bytes_write.sum of push_deposit_kernel<.,COMPACT> per live particle,
 # from the one `ncu --set full` capture of profiles/r01i (6.79 GB + 6.70 GB for 99.8e6 particles)
 NCU_DRAM_BYTES_PER_PARTICLE = 135.2
+# serialised-issue model (profiles/r01e, r01i): per particle 623 FP64 instructions at 2 cycles, 137 of
+# them three-register DFMAs (+1 cycle each), 585 other instructions at 1 cycle, per scheduler
+ISSUE_CYCLES_PER_PARTICLE = 623 * 2 + 137 + 585
 # nominal FP64 pipe: 148 SMs x 64 DFMA lanes/clk x 1.965 GHz (B200)
 FP64_NOMINAL_INSTR_PER_S = 148 * 64 * 1.965e9
 
@@ -315,6 +318,11 @@ def run_ours(args):
         "issue_model_cycles": dict(zip(("dfma_2reg", "dfma_3reg", "dmul", "dmul_plus_3_int"),
                                        ctx.measure_fp64_issue())),
     }
+    # the same launch against the serialised-issue bound: warps per scheduler x cycles per warp
+    sm_hz = 1e6 * ((clocks or {}).get("sm_mhz") or 1965.0)
+    t_issue = ISSUE_CYCLES_PER_PARTICLE * (per_launch / 32.0) / (148 * 4) / sm_hz
+    roofline["issue_model"] = {"cycles_per_particle": ISSUE_CYCLES_PER_PARTICLE, "bound_ms": 1e3 * t_issue,
+                               "frac": t_issue / (pd_ms * 1e-3), "sm_mhz": sm_hz / 1e6}
     # field step: cell-updates/s and HBM fraction (192 B per cell-sweep, N+1 sweeps)
     kernels = {}
     if "field_step" in phases:
