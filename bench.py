@@ -63,7 +63,7 @@ def env_int(k, d):
         return d
 
 
-def parse():
+def parse(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
@@ -80,7 +80,7 @@ def parse():
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
-    return ap.parse_args()
+    return ap.parse_args(argv)
 
 
 class ClockSampler:
@@ -139,7 +139,7 @@ class ClockSampler:
 
 def workload(args, rank):
     """inputs of the chosen config; every rank draws its own particle set (weak scaling)."""
-    from paper_2503_04558_b200 import inputs
+    import inputs
     k = args.config
     n = args.particles or None
     g = args.grid or None
@@ -169,8 +169,13 @@ def run_ours(args):
     rank, world, lrank = env_int("RANK", 0), env_int("WORLD_SIZE", 1), env_int("LOCAL_RANK", 0)
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (libgrpic has no CPU fallback)")
+    if lrank >= torch.cuda.device_count():
+        raise SystemExit("bench.py: rank %d of %d has no GPU (this node has %d)" % (lrank, world, torch.cuda.device_count()))
     torch.cuda.set_device(lrank)
     if world > 1:
+        # communicator lines ("... nranks N ...") on stderr so that a log shows the N ranks
+        os.environ.setdefault("NCCL_DEBUG", "INFO")
+        os.environ.setdefault("NCCL_DEBUG_SUBSYS", "INIT")
         dist.init_process_group("nccl", device_id=torch.device("cuda", lrank))
     K, W = args.steps, max(args.warmup, 3)
 
@@ -190,12 +195,13 @@ def run_ours(args):
     bg = [ctx.to_device(f) for f in cfg["bg"]] if cfg.get("bg") else None
     ctx.fill_guards(fields)
     fields0 = [f.clone() for f in fields]
-    flux = ctx.zeros(3)
+    flux_block = ctx.zeros_block(3)              # one contiguous buffer: ONE all-reduce over ranks
+    flux = list(flux_block.unbind(0))
     cur, alt = grpic.Particles.from_numpy(ptc), grpic.Particles(n)
     n_alive = torch.zeros(W + K + 8, dtype=torch.int64, device="cuda")
     stream = torch.cuda.current_stream()
 
-    names = ("sort", "push_deposit", "finalize", "field_step", "compact")
+    names = ("sort", "push_deposit", "allreduce", "finalize", "field_step", "compact")
     ev = {}
 
     def mark(s, name, which):
@@ -208,8 +214,7 @@ def run_ours(args):
         if sort_every and s % sort_every == 0:
             mark(s, "sort", 0); ctx.sort(cur, alt); mark(s, "sort", 1)
             cur, alt = alt, cur
-        for f in flux:
-            f.zero_()
+        flux_block.zero_()
         mark(s, "push_deposit", 0)
         if fused:       # removal fused into the push: survivors of `cur` are pushed into `alt`
             ctx.push_deposit_compact(cur, alt, fields, flux, dt, n_alive[s:s + 1])
@@ -218,7 +223,7 @@ def run_ours(args):
             ctx.push_deposit(cur, fields, flux, dt)
         mark(s, "push_deposit", 1)
         if world > 1:
-            sharding.allreduce_flux(flux)
+            mark(s, "allreduce", 0); sharding.allreduce_flux(flux_block); mark(s, "allreduce", 1)
         mark(s, "finalize", 0); ctx.finalize_current(flux, filt); mark(s, "finalize", 1)
         mark(s, "field_step", 0); ctx.field_step(fields, flux, dt, bg); mark(s, "field_step", 1)
         if compact and not fused:
@@ -392,7 +397,8 @@ def run_field_only(args):
     Gaussian packet, prescribed random J, damping layer); metric = grid cell-updates per second,
     one cell-update = one full field step (predictor + N correctors + BCs) of one cell."""
     import torch
-    from paper_2503_04558_b200 import grpic, inputs
+    from paper_2503_04558_b200 import grpic
+    import inputs
     torch.cuda.set_device(env_int("LOCAL_RANK", 0))
     if env_int("RANK", 0) != 0:
         return
@@ -529,7 +535,7 @@ def run_reference(args):
     rank = env_int("RANK", 0)
     if rank != 0:
         return
-    from paper_2503_04558_b200 import inputs
+    import inputs
     K, W = args.steps, args.warmup
     budget = 150.0                                     # whole run ends within a few minutes
     n_full = {1: 100_000, 2: 20_000_000, 3: 100_000_000, 5: 200_000_000}[args.config]
@@ -567,11 +573,30 @@ def run_reference(args):
     print(json.dumps(out))
 
 
-if __name__ == "__main__":
-    a = parse()
+def relaunch_argv(argv, gpus, port=None):
+    """command line that starts `gpus` ranks of this script on one node (one process per GPU,
+    rendezvous on 127.0.0.1), as the driver itself launches N > 1."""
+    import socket
+    if port is None:
+        with socket.socket() as so:
+            so.bind(("127.0.0.1", 0))
+            port = so.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(gpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
+def main(argv=None):
+    argv = sys.argv[1:] if argv is None else argv
+    a = parse(argv)
     if a.impl == "reference":
-        run_reference(a)
-    elif a.config == 4:
-        run_field_only(a)
-    else:
-        run_ours(a)
+        return run_reference(a)
+    if a.gpus > 1 and "WORLD_SIZE" not in os.environ and a.config != 4:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves
+        return subprocess.call(relaunch_argv(argv, a.gpus))
+    if a.config == 4:
+        return run_field_only(a)
+    return run_ours(a)
+
+
+if __name__ == "__main__":
+    sys.exit(main() or 0)

@@ -21,7 +21,7 @@ __global__ void tables_1d_kernel(GridDev g, double* r_n, double* r_h, double* dr
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k < g.pitch) {
     const double i = (double)(k - g.i0);
-    r_n[k] = exp(g.xi_in + i * g.dxi);
+    r_n[k] = exp(fma(i, g.dxi, g.xi_in));        // the push recomputes xi_i with this very expression
     r_h[k] = exp(g.xi_in + (i + 0.5) * g.dxi);
     dr_n[k] = exp(g.xi_in + (i + 0.5) * g.dxi) - exp(g.xi_in + (i - 0.5) * g.dxi);
     dr_h[k] = exp(g.xi_in + (i + 1.0) * g.dxi) - exp(g.xi_in + i * g.dxi);

@@ -48,7 +48,7 @@ constexpr int kBlock = GRPIC_PD_BLOCK;
 // no max() (a double fmax costs six instructions for its NaN rules).  No per-slot zero test (each
 // costs a divergent branch around the atomic); issuing all 21 REDs unconditionally is LSU-bound
 // (12.5 ms vs 7.1 ms at 1e8), so the slots that vanish unless a cell face is crossed are grouped.
-__device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t anchor, uint32_t pitch,
+__device__ __forceinline__ void deposit_local(const PolyTab& pt, const grpic_current& J, uint32_t anchor, uint32_t pitch,
                                               double Q, double vphi, double idt, double fxa, double fya,
                                               double fxb, double fyb, bool oax, bool oay, bool obx,
                                               bool oby) {
@@ -65,7 +65,7 @@ __device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t a
   const double Ay0 = hq * (Tb0 + Ta0), Ay1 = hq * (Tb1 + Ta1), Ay2 = hq * (Tb2 + Ta2);
   const double Ax0 = hq * (Sb0 + Sa0), Ax1 = hq * (Sb1 + Sa1), Ax2 = hq * (Sb2 + Sa2);
   // F_phi (Eq.23) = Sb_i U_j + Sa_i V_j
-  const double c3 = vphi * (1.0 / 3.0), c6 = vphi * (1.0 / 6.0);
+  const double c3 = vphi * pt.v[kR3], c6 = vphi * pt.v[kSIXTH];
   const double U0 = fma(c3, Tb0, c6 * Ta0), U1 = fma(c3, Tb1, c6 * Ta1), U2 = fma(c3, Tb2, c6 * Ta2);
   const double V0 = fma(c3, Ta0, c6 * Tb0), V1 = fma(c3, Ta1, c6 * Tb1), V2 = fma(c3, Ta2, c6 * Tb2);
   double* fr = J.Fr + anchor;
@@ -97,7 +97,7 @@ __device__ __forceinline__ void deposit_local(const grpic_current& J, uint32_t a
   }
 }
 
-// ---- TMA (cp.async.bulk) + mbarrier plumbing for the double-buffered particle tiles ----
+// ---- TMA (cp.async.bulk) + mbarrier plumbing for the per-warp particle tile rings ----
 __device__ __forceinline__ uint32_t smem_u32(const void* p) {
   return (uint32_t)__cvta_generic_to_shared(p);
 }
@@ -108,16 +108,20 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
                : "memory");
 }
+// try_wait suspends the warp in hardware up to a system time limit before it returns false: no
+// sleep loop around it (r02a: the NANOSLEEP version executed 14 sleeps + 15 polls per warp tile).
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-  uint32_t ok;
-  do {
-    asm volatile(
-        "{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
-        : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
-        : "memory");
-    if (!ok) __nanosleep(64);                       // do not burn issue slots other warps can use
-  } while (!ok);
+  asm volatile(
+      "{ .reg .pred p;\n"
+      "W: mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@!p bra W; }" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+// one lane of the (converged) warp: the compiler keeps the guarded region on the uniform datapath
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{ .reg .pred P; elect.sync _|P, 0xffffffff; selp.u32 %0, 1, 0, P; }" : "=r"(p));
+  return p != 0;
 }
 // The particle stream (12.8 GB per step at 1e8) is read and written once: it is marked
 // evict-first in L2 so that the field and flux lines the gather and the REDs revisit stay resident.
@@ -135,113 +139,130 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
       : "memory");
 }
 
-// One warp tile of particle input staged in shared memory (structure of arrays, 32 particles).
+// One warp tile of particle input staged in shared memory: structure of arrays, kWTile = 64
+// particles = two 32-particle halves that the warp pushes one after the other (eight 512-byte
+// bulk copies per 64 particles: the issue cost of the staging is halved against 32-particle tiles).
 constexpr int kWarps = kBlock / 32;
+constexpr int kWTile = 64;
 #ifndef GRPIC_PD_STAGES
-#define GRPIC_PD_STAGES 3
+#define GRPIC_PD_STAGES 2
 #endif
-constexpr int kPdStages = GRPIC_PD_STAGES;   // particle tiles in flight per CTA
-struct __align__(128) PtcTile {
-  double x1[kBlock], x2[kBlock], x3[kBlock], u1[kBlock], u2[kBlock], u3[kBlock], w[kBlock];
-  uint32_t flag[kBlock];
-  uint32_t dest[kBlock];   // COMPACT: output index of each particle (written by its own thread, not by TMA)
+constexpr int kPdStages = GRPIC_PD_STAGES;   // particle tiles in flight per warp
+struct __align__(128) WTile {
+  double x1[kWTile], x2[kWTile], x3[kWTile], u1[kWTile], u2[kWTile], u3[kWTile], w[kWTile];
+  uint32_t flag[kWTile];
+  uint32_t ob[4];   // COMPACT: the aligned 16 bytes of `offsets` that hold this tile's two output offsets
 };
-constexpr uint32_t kTileBytes = 7u * kBlock * 8u + kBlock * 4u;
+constexpr uint32_t kTileBytes = 7u * kWTile * 8u + kWTile * 4u;
 
-// Persistent kernel.  A CTA walks the kBlock-particle tiles blockIdx.x, + gridDim.x, ...; a ring of
-// shared-memory stages holds the particle state of the current and the next tiles, each filled by
-// eight 1-D bulk TMA copies (block-uniform addresses: no per-warp address arithmetic).  There is
-// no block-wide barrier in the loop: the warps run independently, each waits on the
-// stage's mbarrier for its data, counts itself out of the stage when it has read it, and the
-// last warp out refills the stage with the tile kPdStages steps ahead.  A warp that takes a slow path
-// (far deposit, large-angle sincos) delays the others by at most one tile.  The last, partial
-// tile (n % kBlock != 0) is staged with plain loads.
+// Persistent kernel, warp-autonomous.  Warp w of the grid walks the 64-particle tiles w, w + W,
+// w + 2W, ... (W = warps in the grid) through its OWN ring of kPdStages shared-memory stages, each
+// filled by eight 1-D bulk TMA copies signalled on the stage's mbarrier.  No block barrier and no
+// coupling between the warps of a CTA: a warp waits only for its own data, which was requested
+// kPdStages - 1 tile times (~10 us) earlier.  Stage hand-back (write-after-read): every lane's
+// shared-memory reads of a stage feed values it has consumed before the __syncwarp() that precedes
+// the refill, __syncwarp() orders the lanes' accesses, and only then does the elected lane issue
+// the bulk copies into that stage (the per-stage "empty" barrier of the usual TMA pipeline,
+// collapsed to a warp barrier because producer and consumers are the same warp).  The last,
+// partial tile (n % 64 != 0) is staged with plain loads.
 //
-// COMPACT: the results are stored to `dst` at offsets[tile] + rank among the tile's live lanes
-// (offsets = exclusive scan of the per-tile live counts of `ptc`), i.e. particles already
-// flagged removed are squeezed out on the way, order preserved; the weight travels along.
+// COMPACT: the results are stored to `dst` at offsets[32-particle tile] + rank among the tile's
+// live lanes (offsets = exclusive scan of the per-tile live counts of `ptc`), i.e. particles
+// already flagged removed are squeezed out on the way, order preserved; the weight travels along.
 // Otherwise dst == ptc and the update is in place.
-template <int MINB, bool COMPACT, int KT>
+template <int MINB, bool COMPACT, int KT, bool TAB>
 __global__ void __launch_bounds__(kBlock, MINB)
 push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
                     const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
-                    int64_t* n_alive, const __grid_constant__ grpic_fields f,
-                    const __grid_constant__ grpic_current J, double dt, int K, uint32_t* status) {
-  __shared__ PtcTile tiles[kPdStages];
-  __shared__ __align__(8) uint64_t full[kPdStages];
-  __shared__ uint32_t done[kPdStages];                       // warps that have finished reading a stage
-  // read once (volatile: the compiler otherwise re-reads SR_TID.X, ~20 cycles each, when short of registers)
+                    const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
+                    const __grid_constant__ PolyTab pt, double dt, int K, uint32_t* status) {
+  __shared__ WTile tiles[kWarps][kPdStages];
+  __shared__ __align__(8) uint64_t full[kWarps][kPdStages];
+  __shared__ uint32_t sdest[COMPACT ? kWarps : 1][kWTile];   // COMPACT: output index of each particle
   uint32_t tid_x;
   asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
-  const int tid = tid_x, lane = tid_x & 31, warp = tid_x >> 5;
+  const uint32_t lane = tid_x & 31u;
+  const uint32_t warp = __shfl_sync(0xffffffffu, tid_x >> 5, 0);   // provably warp-uniform
   // all particle indices fit 32 bits (the C entry rejects n > 0xFFFFFFF0): one-instruction addressing
   const uint32_t n32 = (uint32_t)ptc.n;
-  const uint32_t ntiles = (n32 + kBlock - 1) / kBlock;
-  const uint32_t ntiles32 = (n32 + 31) / 32;           // COMPACT: offsets are per 32-particle tile
-  const uint32_t tstride = gridDim.x;
+  const uint32_t ntiles = (n32 + kWTile - 1) / kWTile;
+  const uint32_t wstride = gridDim.x * kWarps;
+  const uint32_t wtile0 = blockIdx.x * kWarps + warp;
   const double idt = 1.0 / dt;
+  WTile* const ring = tiles[warp];
+  uint64_t* const bars = full[warp];
 
   const uint64_t stream_policy = l2_evict_first_policy();
-  auto issue = [&](uint32_t tile, int stage) {      // one thread; full tiles only
-    const uint32_t k0 = tile * kBlock;
-    if (tile >= ntiles || k0 + kBlock > n32) return;
-    PtcTile& T = tiles[stage];
-    uint64_t* bar = &full[stage];
-    mbar_expect_tx(bar, kTileBytes);
-    tma_load_1d(T.x1, ptc.x1 + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.x2, ptc.x2 + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.x3, ptc.x3 + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.u1, ptc.u1 + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.u2, ptc.u2 + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.u3, ptc.u3 + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.w, ptc.w + k0, kBlock * 8, bar, stream_policy);
-    tma_load_1d(T.flag, ptc.flag + k0, kBlock * 4, bar, stream_policy);
-  };
-  const uint32_t tile0 = blockIdx.x;
-  if (tid == 0) {
-#pragma unroll
-    for (int q = 0; q < kPdStages; ++q) { mbar_init(&full[q], 1); done[q] = 0; }
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-#pragma unroll
-    for (int q = 0; q < kPdStages; ++q) issue(tile0 + q * tstride, q);
-  }
-  __syncthreads();                                  // the only block barrier: before the loop
-
-  int it = 0;
-  // COMPACT: output offset of this warp's 32-particle tile, loaded one tile ahead
-  uint32_t obase_next = (COMPACT && tile0 * kWarps + warp < ntiles32) ? offsets[tile0 * kWarps + warp] : 0u;
-  for (uint32_t tile = tile0; tile < ntiles; tile += tstride, ++it) {
-  const int stage = it % kPdStages;
-  PtcTile& T = tiles[stage];
-  const uint32_t k = tile * kBlock + tid;
-  const uint32_t tile32 = tile * kWarps + warp;     // this warp's 32-particle tile
-  if (tile * kBlock + kBlock <= n32) {
-    mbar_wait(&full[stage], (uint32_t)(it / kPdStages) & 1u);
-  } else {                                          // partial last tile: every thread stages its own slot
-    if (k < n32) {
-      T.x1[tid] = ptc.x1[k]; T.x2[tid] = ptc.x2[k]; T.x3[tid] = ptc.x3[k];
-      T.u1[tid] = ptc.u1[k]; T.u2[tid] = ptc.u2[k]; T.u3[tid] = ptc.u3[k];
-      T.w[tid] = ptc.w[k];
-      T.flag[tid] = ptc.flag[k];
-    } else {
-      T.flag[tid] = 2u;
+  auto issue = [&](uint32_t tile, int stage) {      // whole warp, converged; full tiles only
+    const uint32_t k0 = tile * kWTile;
+    if (tile >= ntiles || k0 + kWTile > n32) return;
+    if (elect_one()) {
+      WTile& T = ring[stage];
+      uint64_t* bar = &bars[stage];
+      mbar_expect_tx(bar, kTileBytes + (COMPACT ? 16u : 0u));
+      // the tile's two output offsets ride along (offsets[2 tile], [2 tile + 1], inside an aligned 16 bytes)
+      if (COMPACT) tma_load_1d(T.ob, offsets + ((2u * tile) & ~3u), 16, bar, stream_policy);
+      tma_load_1d(T.x1, ptc.x1 + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.x2, ptc.x2 + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.x3, ptc.x3 + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.u1, ptc.u1 + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.u2, ptc.u2 + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.u3, ptc.u3 + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.w, ptc.w + k0, kWTile * 8, bar, stream_policy);
+      tma_load_1d(T.flag, ptc.flag + k0, kWTile * 4, bar, stream_policy);
     }
-    __syncwarp();
+  };
+  if (elect_one()) {
+#pragma unroll
+    for (int q = 0; q < kPdStages; ++q) mbar_init(&bars[q], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  const uint32_t flag = T.flag[tid];
-  const bool active = !(flag & 2u);
-  if (COMPACT) {
-    // where this particle's result goes: offsets[tile32] + rank among the live lanes, parked in
-    // the tile's shared memory instead of a register that would live across the whole push
-    const uint32_t live = __ballot_sync(0xffffffffu, active);
-    const uint32_t obase = obase_next;
-    if (tile32 + tstride * kWarps < ntiles32) obase_next = offsets[tile32 + tstride * kWarps];
-    if (tile32 == ntiles32 - 1 && lane == 0) *n_alive = (int64_t)obase + __popc(live);
-    T.dest[tid] = obase + __popc(live & ((1u << lane) - 1u));
+  __syncwarp();
+#pragma unroll
+  for (int q = 0; q < kPdStages; ++q) issue(wtile0 + q * wstride, q);
+
+  // one loop iteration = one 32-particle half of the warp's current 64-particle tile
+  uint32_t tile = wtile0;
+  for (uint32_t j = 0; tile < ntiles; ++j) {
+  const uint32_t half = j & 1u, it = j >> 1;
+  const uint32_t stage = it % kPdStages;
+  WTile& T = ring[stage];
+  if (half == 0) {
+    if (tile * kWTile + kWTile <= n32) {
+      mbar_wait(&bars[stage], (it / kPdStages) & 1u);
+    } else {                                        // partial last tile: every lane stages its own slots
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const uint32_t s2 = h * 32 + lane, k = tile * kWTile + s2;
+        if (k < n32) {
+          T.x1[s2] = ptc.x1[k]; T.x2[s2] = ptc.x2[k]; T.x3[s2] = ptc.x3[k];
+          T.u1[s2] = ptc.u1[k]; T.u2[s2] = ptc.u2[k]; T.u3[s2] = ptc.u3[k];
+          T.w[s2] = ptc.w[k];
+          T.flag[s2] = ptc.flag[k];
+        } else {
+          T.flag[s2] = 2u;
+        }
+      }
+      if (COMPACT && lane < 4) T.ob[lane] = offsets[((2u * tile) & ~3u) + lane];
+      __syncwarp();
+    }
+    if (COMPACT) {
+      // rank of each particle among the live lanes of its 32-particle half, parked in shared
+      // memory instead of registers that would live across the whole push
+      uint32_t lt;
+      asm("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));
+      const uint32_t live0 = __ballot_sync(0xffffffffu, !(T.flag[lane] & 2u));
+      const uint32_t live1 = __ballot_sync(0xffffffffu, !(T.flag[32 + lane] & 2u));
+      sdest[warp][lane] = __popc(live0 & lt);
+      sdest[warp][32 + lane] = __popc(live1 & lt);
+    }
   }
 
-  if (active) {
-    const double x1 = T.x1[tid], x2 = T.x2[tid];
+  {
+  const uint32_t sl = half * 32 + lane;
+  const uint32_t flag = T.flag[sl];
+  if (!(flag & 2u)) {
+    const double x1 = T.x1[sl], x2 = T.x2[sl];
     // species: charge sign of e-/e+; a photon (bit2) feels no Lorentz force
     // (sgn = 0 makes the Boris step the exact identity), has eps = 0 and carries no charge
     const bool photon = (flag & 4u) != 0;
@@ -251,9 +272,14 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     // loads are issued first, exp / sincos / metric run while they are in flight ----
     const double xa = (x1 - g.xi_in) * g.inv_dxi, ya = x2 * g.inv_dth;
     const double fin = floor(xa), fjn = floor(ya);
-    const int ia = (int)fin, ja = (int)fjn;
+    int ia = (int)fin, ja = (int)fjn;
+    // a caller bug (an active particle outside [xi_in, xi_out) x [0, pi]) must not become an
+    // out-of-bounds access: the cell is clamped, the particle flagged removed, nothing deposited
+    const bool offgrid = (uint32_t)ia >= (uint32_t)g.nr || (uint32_t)ja > (uint32_t)g.nth;
+    ia = (int)min((uint32_t)ia, (uint32_t)(g.nr - 1));
+    ja = (int)min((uint32_t)ja, (uint32_t)g.nth);
     const double fih = floor(xa - 0.5), fjh = floor(ya - 0.5);
-    const int ih = (int)fih, jh = (int)fjh;
+    const int ih = offgrid ? ia : (int)fih, jh = offgrid ? ja : (int)fjh;
     const uint32_t bnn = (uint32_t)g.idx(ia, ja), bhn = (uint32_t)g.idx(ih, ja);
     const uint32_t bnh = (uint32_t)g.idx(ia, jh), bhh = (uint32_t)g.idx(ih, jh);
     double G[6][4];
@@ -269,10 +295,19 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       }
     }
 
-    // ---- metric at x^n ----
-    const double r0 = exp(x1);
-    double s0, c0;
-    sincos(x2, &s0, &c0);
+    // ---- r, sin, cos at x^n.  TAB (cells no larger than kSmallStep in xi and theta, i.e. grids of
+    // ~1000 cells and more): from the node tables r_i = exp(xi_i), sin(theta_j), cos(theta_j) that
+    // the field solver uses, times the short series of the in-cell offset; else the full exp / sincos
+    double r0, s0, c0;
+    if (TAB) {
+      const double rn = __ldg(g.r_n + (ia + g.i0));
+      const double sn = __ldg(g.sin_n + (ja + g.j0)), cn = __ldg(g.cos_n + (ja + g.j0));
+      r0 = fma(rn, expm1_small(pt, x1 - fma(fin, g.dxi, g.xi_in)), rn);
+      sincos_shift(pt, sn, cn, x2 - fjn * g.dth, s0, c0);
+    } else {
+      r0 = exp_pt(pt, x1);
+      sincos_pt(pt, x2, s0, c0);
+    }
     const Pos p0 = make_pos(g, r0, s0, c0);
     const double alpha0 = p0.h * rsqrt_nr(p0.h);      // lapse at x^n
 
@@ -297,7 +332,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     }
 
     // ---- Boris (full dt) at x^n ----
-    double ur = T.u1[tid], ut = T.u2[tid], up = T.u3[tid];
+    double ur = T.u1[sl], ut = T.u2[sl], up = T.u3[sl];
     boris(g, p0, alpha0, sgn, dt, D, B, ur, ut, up);
 
     // ---- geodesic predictor + K correctors (Eq.14, 15) ----
@@ -310,9 +345,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 #pragma unroll
     for (int ci = 0; ci < KK; ++ci) {
       double s, c;
-      if (fabs(dth) <= 0.001953125) sincos_shift<true>(s0, c0, dth, s, c);
-      else if (fabs(dth) <= 0.06) sincos_shift<false>(s0, c0, dth, s, c);
-      else sincos(x2 + dth, &s, &c);
+      if (fabs(dth) <= kSmallStep) sincos_shift(pt, s0, c0, dth, s, c);
+      else sincos_pt(pt, x2 + dth, s, c);
       const Pos p1 = make_pos(g, r0 + dr, s, c);
       double Xr, Xt, Xp, Ur, Ut;
       geodesic_rhs(g, p1, photon ? 0.0 : p1.zp1, vr, vt, up, Xr, Xt, Xp, Ur, Ut);
@@ -322,8 +356,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       vr = fma(hdt, Ur + Ur0, ur);
       vt = fma(hdt, Ut + Ut0, ut);
     }
-    const double r = r0 + dr, ph = T.x3[tid] + dph;
-    double th = x2 + dth;
+    const double r = r0 + dr, ph = T.x3[sl] + dph;
+    const double th_dep = x2 + dth;                 // un-reflected new theta: what the deposit sees
 
     // ---- new logical position: ln r = x1 + 2 atanh(dr / (2 r0 + dr)) ----
     double x1n;
@@ -331,111 +365,124 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       const double wq = dr * rcp_nr(r0 + r);
       if (fabs(wq) <= 0.03) {
         const double w2 = wq * wq;
-        double pl = fma(w2, 1.0 / 11.0, 1.0 / 9.0);
-        pl = fma(pl, w2, 1.0 / 7.0);
-        pl = fma(pl, w2, 1.0 / 5.0);
-        pl = fma(pl, w2, 1.0 / 3.0);
+        double pl = fma(w2, pt.v[kR11], pt.v[kR9]);
+        pl = fma(pl, w2, pt.v[kR7]);
+        pl = fma(pl, w2, pt.v[kR5]);
+        pl = fma(pl, w2, pt.v[kR3]);
         const double at = fma(pl * w2, wq, wq);
         x1n = fma(2.0, at, x1);
       } else {
         x1n = log(r);
       }
     }
-    // ---- reflection, removal, new cell ----
-    const double th_dep = th;
-    if (th < 0.0) { th = -th; vt = -vt; }
-    if (th > M_PI) { th = 2.0 * M_PI - th; vt = -vt; }
-    // new logical position (un-reflected), its cell and in-cell fractions
-    const double xb = (x1n - g.xi_in) * g.inv_dxi, yb = th_dep * g.inv_dth;
+    // ---- reflection at the axes: theta -> -theta or 2 pi - theta, u_theta flips ----
+    double th = fabs(th_dep);
+    // sign bit of th_dep moves into u_theta (th_dep < 0 flips it)
+    vt = __hiloint2double(__double2hiint(vt) ^ (__double2hiint(th_dep) & 0x80000000), __double2loint(vt));
+    bool reflected = __double2hiint(th_dep) < 0;
+    if (th > pt.v[kPI]) { th = pt.v[kTWOPI] - th; vt = -vt; reflected = true; }
+    // ---- new position in index space.  The deposit takes the PRODUCT form (x - xi_in) * (1/dxi): it
+    // is the expression the next step (and the rho deposit) applies to the stored position, so the
+    // charge a particle leaves at its new position is exactly the charge it starts from.  The cell
+    // index is the floor of the correctly rounded QUOTIENT (the oracle's division): the product
+    // refined by one residual step, q + (a - q d)(1/d), equals the IEEE division whenever 1/d is
+    // correctly rounded, which the host guarantees ----
+    const double ax = x1n - g.xi_in;
+    const double xb = ax * g.inv_dxi, yb = th_dep * g.inv_dth;
     const double fib = floor(xb), fjb = floor(yb);
     const int ib = (int)fib, jb = (int)fjb;
     const double fxb = xb - fib, fyb = yb - fjb;
+    const int icq = (int)floor(fma(fma(-xb, g.dxi, ax), g.inv_dxi, xb));
+    const int jcq = (int)floor(fma(fma(-yb, g.dth, th_dep), g.inv_dth, yb));
+    // finite test on the three quantities that reach the grid (a non-finite momentum alone shows
+    // up in the position one step later): the high words, read as floats, are finite floats
+    // unless the double is inf / nan or >= 2^1017
+    const bool finite = fabsf(__int_as_float(__double2hiint(x1n))) + fabsf(__int_as_float(__double2hiint(th_dep))) +
+                            fabsf(__int_as_float(__double2hiint(dph))) < __int_as_float(0x7f800000);
+    const bool out = !(x1n >= g.xi_in && x1n < g.xi_out) || offgrid || !finite;
     uint32_t nflag = flag, ncell;
-    const bool finite = isfinite(x1n) && isfinite(th) && isfinite(ph) && isfinite(vr) && isfinite(vt);
-    const bool out = !finite || (x1n < g.xi_in) || (x1n >= g.xi_out);
     if (out) {
       nflag |= 2u;
       ncell = 0xFFFFFFFFu;
-      if (!finite && status) atomicOr(status, GRPIC_STATUS_NONFINITE);
+      if (status && (!finite || offgrid))
+        atomicOr(status, offgrid ? GRPIC_STATUS_OFFGRID : GRPIC_STATUS_NONFINITE);
     } else {
-      // cell = floor of the quotient; the product form decides unless it is within 1e-7 of
-      // a cell edge, where the quotient itself is taken (same decision as a division)
-      int ic = ib, jc = jb;
-      if (fabs(fxb - 0.5) > 0.5 - 1e-7) ic = (int)floor((x1n - g.xi_in) / g.dxi);
-      if (th != th_dep) {                             // reflected at an axis: recompute in theta
-        const double cy = th * g.inv_dth, fc = floor(cy);
-        jc = (int)fc;
-        if (fabs(cy - fc - 0.5) > 0.5 - 1e-7) jc = (int)floor(th / g.dth);
-      } else if (fabs(fyb - 0.5) > 0.5 - 1e-7) {
-        jc = (int)floor(th / g.dth);
+      int jc = jcq;
+      if (reflected) {                              // at an axis: the cell of the mirrored theta
+        double yc = th * g.inv_dth;
+        yc = fma(fma(-yc, g.dth, th), g.inv_dth, yc);
+        jc = (int)floor(yc);
       }
-      ic = min(max(ic, 0), g.nr - 1);
+      const int ic = min(max(icq, 0), g.nr - 1);
       jc = min(max(jc, 0), g.nth - 1);
       ncell = (uint32_t)(jc * g.nr + ic);
     }
-    const uint32_t kd = COMPACT ? T.dest[tid] : k;
+    // COMPACT: output index = offsets[this 32-particle half] + rank among its live lanes
+    const uint32_t kd = COMPACT ? T.ob[(tile & 1u) * 2u + half] + sdest[warp][sl] : tile * kWTile + sl;
     __stcs(dst.x1 + kd, x1n); __stcs(dst.x2 + kd, th); __stcs(dst.x3 + kd, ph);   // streaming stores
     __stcs(dst.u1 + kd, vr); __stcs(dst.u2 + kd, vt); __stcs(dst.u3 + kd, up);
-    if (COMPACT) __stcs(dst.w + kd, T.w[tid]);
+    if (COMPACT) __stcs(dst.w + kd, T.w[sl]);
     __stcs(dst.cell + kd, ncell);
     __stcs(dst.flag + kd, nflag);
 
     // ---- deposit: 3x3 window anchored at the lower of the old / new cell ----
-    if (finite && !photon) {
-      const double q = sgn * T.w[tid];
+    if (finite && !photon && !offgrid) {
+      const double q = sgn * T.w[sl];
       const double vph = q * dph * idt;
       const int di = ib - ia, dj = jb - ja;
-      if (di >= -1 && di <= 1 && dj >= -1 && dj <= 1) {
+      if ((uint32_t)(di + 1) <= 2u && (uint32_t)(dj + 1) <= 2u) {
         const int iw = min(ia, ib), jw = min(ja, jb);
-        deposit_local(J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - fin, ya - fjn, fxb,
+        deposit_local(pt, J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - fin, ya - fjn, fxb,
                       fyb, ia != iw, ja != jw, ib != iw, jb != jw);
       } else {
         deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
       }
     }
   }
-  // this warp is done with the stage; the last warp out refills it with the tile two steps ahead
-  __syncwarp();
-  if (lane == 0) {
-    if (atomicAdd(&done[stage], 1u) == kWarps - 1) {
-      atomicExch(&done[stage], 0u);
-      issue(tile + kPdStages * tstride, stage);
-    }
+  }
+  if (half == 1) {       // this warp is done with the stage: refill it with the tile kPdStages steps ahead
+    __syncwarp();
+    issue(tile + kPdStages * wstride, stage);
+    tile += wstride;
   }
   }
 }
 
-template <int MINB, bool COMPACT, int KT>
+template <int MINB, bool COMPACT, int KT, bool TAB>
 int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
-                        const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
+                        const uint32_t* offsets, const grpic_fields& f,
                         const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
   static int per_sm = 0;   // resident CTAs per SM of this instantiation
   if (per_sm == 0) {
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, COMPACT, KT>,
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, COMPACT, KT, TAB>,
                                                       kBlock, 0) != cudaSuccess || per_sm < 1)
       per_sm = 1;
   }
-  const int64_t nblocks = (ptc.n + kBlock - 1) / kBlock;
+  const int64_t nblocks = (ptc.n + kWarps * kWTile - 1) / (kWarps * kWTile);
   const int64_t resident = (int64_t)ctx->sm_count * per_sm;
   const unsigned grid = (unsigned)(nblocks < resident ? nblocks : resident);
-  push_deposit_kernel<MINB, COMPACT, KT><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, n_alive, f, J,
-                                                                  dt, ctx->p.geo_iters, status);
+  push_deposit_kernel<MINB, COMPACT, KT, TAB><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, f, J, kPolyTabHost, dt,
+                                                                  ctx->p.geo_iters, status);
   return grpic_launch_ok();
 }
 
 template <bool COMPACT>
 int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
-                          const uint32_t* offsets, int64_t* n_alive, const grpic_fields& f,
+                          const uint32_t* offsets, const grpic_fields& f,
                           const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
   // tuning knob (read once): GRPIC_PD_MINB=4 selects the 126-register build (GRPIC_PD_MA CTAs per
   // SM), anything else the 96-register one (GRPIC_PD_MB); defaults: compacting -> 126, in place -> 96
   static int minb = -1;
   if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : (COMPACT ? 4 : 5); }
+  // TAB: cells small enough for the node-table + in-cell series form of r, sin, cos (push_math.cuh)
+  const bool tab = ctx->g.dxi <= kSmallStep && ctx->g.dth <= kSmallStep;
   if (ctx->p.geo_iters != 3)
-    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 0>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 0, false>(ctx, ptc, dst, offsets, f, J, dt, status, st);
+  if (!tab)
+    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 3, false>(ctx, ptc, dst, offsets, f, J, dt, status, st);
   if (minb == 4)
-    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
-  return launch_push_deposit<GRPIC_PD_MB, COMPACT, 3>(ctx, ptc, dst, offsets, n_alive, f, J, dt, status, st);
+    return launch_push_deposit<GRPIC_PD_MA, COMPACT, 3, true>(ctx, ptc, dst, offsets, f, J, dt, status, st);
+  return launch_push_deposit<GRPIC_PD_MB, COMPACT, 3, true>(ctx, ptc, dst, offsets, f, J, dt, status, st);
 }
 
 // live particles per 32-particle tile: each thread reads four flags (16 bytes), eight threads
@@ -454,9 +501,21 @@ __global__ void __launch_bounds__(256) tile_live_kernel(const uint32_t* flag, in
   c += __shfl_xor_sync(0xffffffffu, c, 4);
   if ((threadIdx.x & 7) == 0 && k < n) counts[k >> 5] = c;
 }
-// out[k] for k in [*n_alive, n): flag = removed
-__global__ void mark_tail_range_kernel(grpic_particles out, int64_t n, const int64_t* n_alive) {
-  for (int64_t k = *n_alive + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n;
+// survivor count = offsets[last 32-particle tile] + its live lanes (every CTA recomputes it from the
+// input flags; CTA 0 publishes it), then out[k] for k in [n_alive, n): flag = removed
+__global__ void __launch_bounds__(256) finish_compact_kernel(grpic_particles out, const uint32_t* in_flag, int64_t n,
+                                                             const uint32_t* offsets, int64_t* n_alive) {
+  __shared__ int64_t na_s;
+  if (threadIdx.x < 32) {
+    const int64_t last = (n - 1) >> 5, k = last * 32 + threadIdx.x;
+    const uint32_t live = __ballot_sync(0xffffffffu, k < n && !(in_flag[k] & 2u));
+    if (threadIdx.x == 0) {
+      na_s = (int64_t)offsets[last] + __popc(live);
+      if (blockIdx.x == 0) *n_alive = na_s;
+    }
+  }
+  __syncthreads();
+  for (int64_t k = na_s + (int64_t)blockIdx.x * blockDim.x + threadIdx.x; k < n;
        k += (int64_t)gridDim.x * blockDim.x) {
     out.flag[k] = 2u;
     out.cell[k] = 0xFFFFFFFFu;
@@ -484,7 +543,7 @@ extern "C" int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const gr
   if (!tma_aligned(ptc)) return GRPIC_ERR_ARG;
   if (ptc->n == 0) return GRPIC_OK;
   if (ptc->n > 0xFFFFFFF0LL) return GRPIC_ERR_ARG;
-  const int rc = dispatch_push_deposit<false>(ctx, *ptc, *ptc, nullptr, nullptr, *fields, *flux, dt, status,
+  const int rc = dispatch_push_deposit<false>(ctx, *ptc, *ptc, nullptr, *fields, *flux, dt, status,
                                               (cudaStream_t)stream);
   grpic_count_launches(1);
   return rc;
@@ -511,9 +570,9 @@ extern "C" int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles*
   tile_live_kernel<<<(unsigned)((n + 1023) / 1024), 256, 0, st>>>(in->flag, n, offsets);
   int rc = grpic_exclusive_scan(offsets, ntiles, offsets + ntiles, st);
   if (rc != GRPIC_OK) return rc;
-  rc = dispatch_push_deposit<true>(ctx, *in, *out, offsets, n_alive, *fields, *flux, dt, status, st);
+  rc = dispatch_push_deposit<true>(ctx, *in, *out, offsets, *fields, *flux, dt, status, st);
   if (rc != GRPIC_OK) return rc;
-  mark_tail_range_kernel<<<ctx->sm_count, 256, 0, st>>>(*out, n, n_alive);
+  finish_compact_kernel<<<ctx->sm_count, 256, 0, st>>>(*out, in->flag, n, offsets, n_alive);
   grpic_count_launches(3);
   return grpic_launch_ok();
 }

@@ -7,8 +7,63 @@
 #include <math.h>
 
 #include "grpic_internal.cuh"
+#include "poly_tables.cuh"
 
 namespace {
+
+// ---- the kernel's own exp / sincos: the algorithms of any libm (Cody-Waite reduction with a
+// round-to-nearest magic constant, Horner polynomials), coefficients from the PolyTab kernel
+// parameter (one LDCU each; a literal costs two UMOV on sm_100a), no special-case branches: arguments
+// are ln r in [xi_in, xi_out] and theta near [0, pi]; anything else (NaN, huge) yields a
+// non-finite or meaningless value that the caller's removal test catches.  Errors < 1 ulp.
+constexpr double kMagic = 6755399441055744.0;        // 1.5 * 2^52: x + kMagic rounds x to an integer
+__device__ __forceinline__ double exp_pt(const PolyTab& pt, double x) {
+  const double t = fma(x, pt.v[kL2E], kMagic);
+  const int n = __double2loint(t);
+  const double fn = t - kMagic;
+  double r = fma(fn, -pt.v[kLN2_HI], x);
+  r = fma(fn, -pt.v[kLN2_LO], r);
+  double p = pt.v[kEXP0];
+  p = fma(p, r, pt.v[kEXP1]);
+  p = fma(p, r, pt.v[kEXP2]);
+  p = fma(p, r, pt.v[kEXP3]);
+  p = fma(p, r, pt.v[kEXP4]);
+  p = fma(p, r, pt.v[kEXP5]);
+  p = fma(p, r, pt.v[kEXP6]);
+  p = fma(p, r, pt.v[kEXP7]);
+  p = fma(p, r, pt.v[kEXP8]);
+  p = fma(p, r, pt.v[kEXP9]);
+  p = fma(p, r, 0.5);
+  p = fma(p, r, 1.0);
+  p = fma(p, r, 1.0);                                 // exp(r), |r| <= ln2/2
+  return __hiloint2double(__double2hiint(p) + (n << 20), __double2loint(p));   // * 2^n
+}
+__device__ __forceinline__ void sincos_pt(const PolyTab& pt, double x, double& s, double& c) {
+  const double t = fma(x, pt.v[kTWO_OVER_PI], kMagic);
+  const int q = __double2loint(t);
+  const double fk = t - kMagic;
+  double r = fma(fk, -pt.v[kPIO2_1], x);
+  r = fma(fk, -pt.v[kPIO2_2], r);
+  r = fma(fk, -pt.v[kPIO2_3], r);                      // |r| <= pi/4
+  const double z = r * r;
+  double ps = fma(pt.v[kSIN0], z, pt.v[kSIN1]);
+  double pc = fma(pt.v[kCOS0], z, pt.v[kCOS1]);
+  ps = fma(ps, z, pt.v[kSIN2]);
+  pc = fma(pc, z, pt.v[kCOS2]);
+  ps = fma(ps, z, pt.v[kSIN3]);
+  pc = fma(pc, z, pt.v[kCOS3]);
+  ps = fma(ps, z, pt.v[kSIN4]);
+  pc = fma(pc, z, pt.v[kCOS4]);
+  ps = fma(ps, z, pt.v[kSIN5]);
+  pc = fma(pc, z, pt.v[kCOS5]);
+  const double sr = fma(ps * z, r, r);                // sin r
+  const double cr = fma(pc * z, z, fma(z, -0.5, 1.0));   // cos r
+  // quadrant q mod 4: (sin, cos) = (sr, cr), (cr, -sr), (-sr, -cr), (-cr, sr)
+  const bool odd = (q & 1) != 0;
+  const double sa = odd ? cr : sr, ca = odd ? sr : cr;
+  s = __hiloint2double(__double2hiint(sa) ^ ((q << 30) & 0x80000000), __double2loint(sa));
+  c = __hiloint2double(__double2hiint(ca) ^ (((q + 1) << 30) & 0x80000000), __double2loint(ca));
+}
 
 // 1/x: MUFU.RCP64H seed (relative error <= 2^-23, PTX rcp.approx.ftz.f64) + ONE third-order step
 // y (1 + e + e^2), e = 1 - x y: error ~ e^3 = 2^-69, three FMAs instead of the four of two Newton
@@ -25,7 +80,7 @@ __device__ __forceinline__ double rsqrt_nr(double x) {
   asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
   const double h = 0.5 * x;
   const double e = fma(-(h * y), y, 0.5);
-  return fma(y, fma(e, 1.5, 1.0) * e, y);
+  return fma(y, fma(e * 1.5, e, e), y);               // immediates only: no constant register pair
 }
 
 struct Pos {          // position-only terms at (r, theta)
@@ -174,29 +229,28 @@ __device__ __forceinline__ void red_add(double* p, double v) {
       "d"(v)
       : "memory");
 }
-// sin, cos of th0 + d from (s0, c0) for |d| <= 0.06 (angle addition, Taylor in d).  SHORT:
-// |d| <= 2^-9, where two terms less of each series are exact to < 1e-19 (the step of a particle
-// is dt X^theta <= dt / rho: at the production time steps every corrector takes this path).
-template <bool SHORT>
-__device__ __forceinline__ void sincos_shift(double s0, double c0, double d, double& s, double& c) {
+// Short series for steps |d| <= kSmallStep = 2^-8 (the dropped terms are < 1e-18 relative): the
+// in-cell offset of a particle on grids of ~1000 cells and more, and dt X^theta <= dt / rho of every
+// corrector at the production time steps.  Both share the four Taylor coefficients -1/6, 1/120,
+// -1/24, 1/720.
+constexpr double kSmallStep = 0.00390625;
+// sin, cos of th0 + d from (s0, c0) by angle addition
+__device__ __forceinline__ void sincos_shift(const PolyTab& pt, double s0, double c0, double d, double& s, double& c) {
   const double d2 = d * d;
-  double ps, pc;
-  if (SHORT) {
-    ps = fma(d2, 1.0 / 120.0, -1.0 / 6.0);
-    pc = fma(fma(d2, 1.0 / 720.0, -1.0 / 24.0), d2, 0.5);
-  } else {
-    ps = fma(d2, 1.0 / 362880.0, -1.0 / 5040.0);
-    ps = fma(ps, d2, 1.0 / 120.0);
-    ps = fma(ps, d2, -1.0 / 6.0);
-    pc = fma(d2, 1.0 / 3628800.0, -1.0 / 40320.0);
-    pc = fma(pc, d2, 1.0 / 720.0);
-    pc = fma(pc, d2, -1.0 / 24.0);
-    pc = fma(pc, d2, 0.5);
-  }
+  const double ps = fma(d2, pt.v[kR120], pt.v[kR6]);
+  const double pc = fma(fma(d2, pt.v[kR720], pt.v[kR24]), d2, 0.5);
   const double sd = fma(ps * d2, d, d);                         // sin d
   const double vd = pc * d2;                                    // 1 - cos d
   s = s0 + fma(c0, sd, -s0 * vd);
   c = c0 - fma(s0, sd, c0 * vd);
+}
+// exp(d) - 1 = sinh d + (cosh d - 1): the same two polynomials evaluated at -d^2
+__device__ __forceinline__ double expm1_small(const PolyTab& pt, double d) {
+  const double m = -d * d;
+  const double ps = fma(m, pt.v[kR120], pt.v[kR6]);
+  const double pc = fma(fma(m, pt.v[kR720], pt.v[kR24]), m, 0.5);
+  const double sh = fma(ps * m, d, d);                          // sinh d
+  return fma(-pc, m, sh);                                       // + cosh d - 1
 }
 
 // General-window deposit (moves of more than one cell; never taken below the Courant limit).

@@ -182,6 +182,11 @@ class Context:
         z = [torch.zeros(self.rows, self.pitch, dtype=torch.float64, device="cuda") for _ in range(n)]
         return z if n > 1 else z[0]
 
+    def zeros_block(self, n):
+        """n grid arrays in ONE contiguous allocation [n, rows, pitch] (block[k] is array k): the
+        three flux arrays of a multi-GPU run are summed over ranks with a single all-reduce."""
+        return torch.zeros(n, self.rows, self.pitch, dtype=torch.float64, device="cuda")
+
     def to_device(self, arr):
         t = torch.zeros(self.rows, self.pitch, dtype=torch.float64, device="cuda")
         G = self.ng

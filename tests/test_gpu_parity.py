@@ -7,7 +7,7 @@ import os
 import numpy as np
 import pytest
 
-from paper_2503_04558_b200 import inputs
+import inputs
 
 pytestmark = pytest.mark.gpu
 

@@ -11,7 +11,8 @@ import numpy as np
 import pytest
 
 from paper_2503_04558_b200 import build as grpic_build
-from paper_2503_04558_b200 import inputs, sharding
+import inputs
+from paper_2503_04558_b200 import sharding
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
@@ -78,7 +79,8 @@ import os, sys
 sys.path.insert(0, %(root)r)
 import numpy as np, torch, torch.distributed as dist
 import oracle
-from paper_2503_04558_b200 import inputs, sharding
+import inputs
+from paper_2503_04558_b200 import sharding
 dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%(port)d", rank=int(sys.argv[1]), world_size=2)
 cfg = inputs.config(1, nr=24, nth=20, n=600)
 p, dt, ptc = cfg["params"], cfg["dt"], cfg["particles"]

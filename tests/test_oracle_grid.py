@@ -8,7 +8,7 @@ import pytest
 import scipy.integrate
 
 import oracle
-from paper_2503_04558_b200 import inputs
+import inputs
 
 
 def small_params(nr=24, nth=20, a=0.9, **kw):

@@ -7,7 +7,7 @@ import numpy as np
 import pytest
 
 import oracle
-from paper_2503_04558_b200 import inputs
+import inputs
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 
@@ -293,7 +293,7 @@ def test_photon_species_push_ignores_fields_and_moves_at_light_speed():
     Flat space (M = 0): a photon follows a straight line at unit speed whatever |u| is
     (closed form), and its energy |u| is conserved; pins eps = 0 (a massive particle with the
     same u would move at |u|/sqrt(1+u^2) < 1)."""
-    from paper_2503_04558_b200 import inputs
+    import inputs
     p = inputs.grid_params(32, 32, 0.0, r_out=40.0, r_in=2.0, M=0.0)
     strong = [np.full(inputs.grid_shape(p), 3.0) for _ in range(6)]
     zero = [np.zeros(inputs.grid_shape(p)) for _ in range(6)]
@@ -336,7 +336,7 @@ def test_photon_species_push_ignores_fields_and_moves_at_light_speed():
 
 
 def test_photons_carry_no_current_and_no_charge():
-    from paper_2503_04558_b200 import inputs
+    import inputs
     p = inputs.grid_params(24, 20, 0.9)
     ptc = inputs.make_particles(p, 400, 3, "logical", ("loguniform", 0.1, 10.0))
     fields = inputs.analytic_fields(p, "monopole")
@@ -381,7 +381,7 @@ def test_pair_production_conserves_fido_momentum_and_energy():
     energy is eps_ph and only leptons with Gamma >= gamma_thr emit; conversion: a fraction
     p_convert of the photons (Eq.26), the two leptons share the photon's FIDO energy, all momenta
     parallel; children appended in parent order with position, cell and weight of the parent."""
-    from paper_2503_04558_b200 import inputs
+    import inputs
     p = inputs.grid_params(32, 32, 0.9)
     n = 6000
     ptc = inputs.make_particles(p, n, 9, "logical", ("loguniform", 1.0, 1e3))
@@ -498,7 +498,7 @@ def test_vay_pure_B_conserves_energy_and_matches_boris_to_second_order():
 
 
 def test_push_with_vay_option_uses_vay():
-    from paper_2503_04558_b200 import inputs
+    import inputs
     p = inputs.grid_params(24, 20, 0.9)
     fields = inputs.analytic_fields(p, "wald")
     ptc = inputs.make_particles(p, 50, 3, "logical", ("loguniform", 0.1, 10.0))
