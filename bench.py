@@ -75,8 +75,15 @@ def parse(argv=None):
     ap.add_argument("--sort-every", type=int, default=-1)
     ap.add_argument("--e2e-steps", type=int, default=3)
     ap.add_argument("--e2e-chunk", type=int, default=0, help="particles per chunk of grpic_step_host (0 = library default)")
-    ap.add_argument("--separate-compact", action="store_true",
-                    help="run compaction as its own pass instead of fused into the push")
+    ap.add_argument("--compaction", default="sort", choices=["sort", "fused", "separate"],
+                    help="how removed particles leave the arrays (configs with removal): 'sort' = the push only "
+                         "flags them, the periodic cell sort moves them behind the live ones (default); 'fused' = "
+                         "order-preserving compaction fused into every push; 'separate' = its own pass every step")
+    ap.add_argument("--separate-compact", action="store_true", help="alias of --compaction separate")
+    ap.add_argument("--sort-order", default="interleaved", choices=["interleaved", "stable"],
+                    help="cell sort order: rank-interleaved inside blocks of --sort-block cells "
+                         "(grpic_sort_interleaved, contention-free deposit) or the plain stable order (grpic_sort)")
+    ap.add_argument("--sort-block", type=int, default=8)
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -188,7 +195,11 @@ def run_ours(args):
     sort_every = args.sort_every if args.sort_every >= 0 else (meta.get("sort_every") or 20)
     compact = bool(meta.get("compact_every", 0))
     filt = int(meta.get("filter_passes", 0))
-    fused = compact and not args.separate_compact
+    policy = "separate" if args.separate_compact else args.compaction
+    if not compact:
+        policy = "none"
+    fused = policy == "fused"
+    lazy = policy == "sort"
 
     ctx = grpic.Context(p, n)
     fields = [ctx.to_device(f) for f in cfg["fields"]]
@@ -199,6 +210,7 @@ def run_ours(args):
     flux = list(flux_block.unbind(0))
     cur, alt = grpic.Particles.from_numpy(ptc), grpic.Particles(n)
     n_alive = torch.zeros(W + K + 8, dtype=torch.int64, device="cuda")
+    removed = torch.zeros(W + K + 8, dtype=torch.int64, device="cuda")   # lazy removal: particles flagged per step
     stream = torch.cuda.current_stream()
 
     names = ("sort", "push_deposit", "allreduce", "finalize", "field_step", "compact")
@@ -212,7 +224,12 @@ def run_ours(args):
     def step(s, state):
         cur, alt = state
         if sort_every and s % sort_every == 0:
-            mark(s, "sort", 0); ctx.sort(cur, alt); mark(s, "sort", 1)
+            mark(s, "sort", 0)
+            if args.sort_order == "interleaved":
+                ctx.sort_interleaved(cur, alt, args.sort_block)
+            else:
+                ctx.sort(cur, alt)
+            mark(s, "sort", 1)
             cur, alt = alt, cur
         flux_block.zero_()
         mark(s, "push_deposit", 0)
@@ -220,13 +237,15 @@ def run_ours(args):
             ctx.push_deposit_compact(cur, alt, fields, flux, dt, n_alive[s:s + 1])
             cur, alt = alt, cur
         else:
+            if lazy:
+                ctx.set_removed_counter(removed[s:s + 1])
             ctx.push_deposit(cur, fields, flux, dt)
         mark(s, "push_deposit", 1)
         if world > 1:
             mark(s, "allreduce", 0); sharding.allreduce_flux(flux_block); mark(s, "allreduce", 1)
         mark(s, "finalize", 0); ctx.finalize_current(flux, filt); mark(s, "finalize", 1)
         mark(s, "field_step", 0); ctx.field_step(fields, flux, dt, bg); mark(s, "field_step", 1)
-        if compact and not fused:
+        if policy == "separate":
             mark(s, "compact", 0); ctx.compact(cur, alt, n_alive[s:s + 1]); mark(s, "compact", 1)
             cur, alt = alt, cur
         return cur, alt
@@ -266,7 +285,11 @@ def run_ours(args):
         sampler.stop()
 
     # particles actually pushed per timed step (alive at the start of the step)
-    if compact:
+    if lazy:
+        ctx.set_removed_counter(None)
+        gone = np.concatenate([[0], np.cumsum(removed.cpu().numpy())])
+        pushed = [int(n - gone[s]) for s in range(W, W + K)]
+    elif compact:
         al = n_alive.cpu().numpy()
         pushed = [int(al[s]) if fused else (n if s == 0 else int(al[s - 1])) for s in range(W, W + K)]
     else:
@@ -284,6 +307,8 @@ def run_ours(args):
         if ts:
             phases[nm] = {"ms_per_call": float(np.mean(ts)), "calls": len(ts),
                           "ms_per_step": float(np.sum(ts) / K)}
+            if nm == "push_deposit":      # the sawtooth between two cell sorts (step index mod sort_every)
+                phases[nm]["per_step_ms"] = [round(float(t), 3) for t in ts]
     status = int(ctx.status.item())
 
     # ---- sustained FP64 pipe rate (same clocks regime as the long step), then rooflines
@@ -373,9 +398,15 @@ def run_ours(args):
             "config": {"workload": "BASELINE.json configs[%d]: %dx%d (log r, theta) grid, a=%.2f, "
                                    "%d particles per GPU" % (args.config - 1, p["nr"], p["nth"], p["a"], n),
                        "particles_per_gpu": n, "grid": [p["nr"], p["nth"]], "dt": dt,
-                       "sort_every": sort_every, "compact_every_step": compact,
-                       "compaction": ("fused into the push (grpic_push_deposit_compact)" if fused else
-                                      "separate pass (grpic_compact)") if compact else "none",
+                       "sort_every": sort_every,
+                       "sort_order": ("rank-interleaved inside blocks of %d cells (grpic_sort_interleaved)"
+                                      % args.sort_block) if args.sort_order == "interleaved" else "stable (grpic_sort)",
+                       "compact_every_step": policy in ("fused", "separate"),
+                       "compaction": {"sort": "removed particles are flagged by the push and skipped; the cell sort "
+                                              "moves them behind the live ones every %d steps" % sort_every,
+                                      "fused": "fused into every push (grpic_push_deposit_compact)",
+                                      "separate": "separate pass every step (grpic_compact)",
+                                      "none": "none"}[policy],
                        "filter_passes": filt,
                        "field_step": True, "field_iters": p["field_iters"], "geo_iters": p["geo_iters"],
                        "macro_weight": BENCH_WEIGHT,

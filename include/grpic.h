@@ -114,6 +114,15 @@ int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes);
 int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                        grpic_current* flux, double dt, uint32_t* status, void* stream);
 
+/* Lazy removal: grpic_push_deposit only FLAGS the particles that leave; they are
+ * skipped by every later call and moved behind the live particles by the next grpic_sort /
+ * grpic_sort_interleaved (their key is the largest), so a caller that sorts periodically needs no
+ * compaction pass.  To know the survivor count without a pass over the flags, hand the library a
+ * DEVICE counter: every grpic_push_deposit / grpic_push_deposit_compact call adds to *counter the
+ * number of particles it flagged removed (NULL, the default, disables it).  The counter is the
+ * caller's memory; the library keeps only the pointer until it is replaced. */
+int grpic_set_removed_counter(grpic_ctx* ctx, unsigned long long* device_counter);
+
 /* The same particle step with the THIRD-ORDER (cubic B-spline) shape, the paper's configuration
  * option ("a third order spline is also available"): gather over the 4 x 4 nodes of
  * the spline's support on each component's own lattice, prefix-sum deposit (Eq.21-23) over the
@@ -209,6 +218,18 @@ int grpic_circulation(grpic_ctx* ctx, const grpic_fields* fields, double* const 
 /* Stable sort by key = removed ? ncells : cell.  `out` receives the reordered SoA (must not
  * alias `in`), `perm[k]` = source index of output k (may be NULL).  out->n = in->n. */
 int grpic_sort(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, uint32_t* perm, void* stream);
+
+/* Cell sort in the contention-free order (BASELINE.json north_star: "deposition ... keyed by sorted
+ * cell", "heavy atomic contention"; not in the paper).  Order = lexicographic (cell / block_cells,
+ * rank, cell % block_cells), where rank is the position of the particle among the particles of
+ * its cell in the stable order of grpic_sort; removed particles follow in their input order.
+ * All keys are distinct, so the permutation is unique (bit-exact against the oracle).  Particles
+ * that are neighbours in memory then sit in different, adjacent cells: the lanes of a warp of
+ * grpic_push_deposit never add to one address in one RED instruction.  block_cells: power of two
+ * in [1, 32] (1 = the order of grpic_sort; 8 is the measured best).  Same arguments, ownership and
+ * errors as grpic_sort; the workspace must come from grpic_workspace_bytes. */
+int grpic_sort_interleaved(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, uint32_t* perm,
+                           int32_t block_cells, void* stream);
 
 /* Order-preserving removal of flagged particles: survivors are copied to `out` (must not
  * alias `in`) in order; their count is written to the DEVICE word n_alive. */

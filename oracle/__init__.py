@@ -252,6 +252,14 @@ def sort(cell, flag):
     return perm
 
 
+def sort_interleaved(cell, flag, ncells, block_cells):
+    n = len(cell)
+    perm = np.zeros(n, dtype=np.uint32)
+    lib().orc_sort_interleaved(C.c_int64(n), _u(cell), _u(flag), C.c_uint32(ncells), C.c_uint32(block_cells),
+                               _u(perm))
+    return perm
+
+
 def compact(flag):
     n = len(flag)
     idx = np.zeros(n, dtype=np.uint32)

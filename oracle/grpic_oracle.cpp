@@ -21,6 +21,7 @@
 //   orc_circulation/field div B exactly preserved; div D - rho preserved; Wald/monopole
 //                         stationarity ~ Delta^2; Heun limit / order in dt
 //   orc_sort/orc_compact  = std::stable_sort / order-preserving filter (library definition)
+//   orc_sort_interleaved  numpy lexsort of the defining tuple; hand-built example; B = 1 reduces to orc_sort
 //   shape option 3        cubic B-spline: partition of unity, moments, C2 knots; continuity to
 //                         round-off with the spline in rho and fluxes; exact gather of linear fields
 //   orc_philox4x32_10     the published known-answer vectors (tests/golden/philox4x32_10.txt)
@@ -944,6 +945,32 @@ void orc_sort(int64_t n, const uint32_t* cell, const uint32_t* flag, uint32_t* p
   for (int64_t k = 0; k < n; ++k) key[k] = (flag[k] & 2u) ? 0xFFFFFFFFu : cell[k];
   std::iota(perm, perm + n, 0u);
   std::stable_sort(perm, perm + n, [&](uint32_t x, uint32_t y) { return key[x] < key[y]; });
+}
+
+// S11b (not in the paper; BASELINE.json north_star "deposition ... keyed by sorted cell", DESIGN.md
+// reading S11b): the contention-free cell order.  With rank = position of a particle among the
+// particles of its cell in the stable order of S11, live particles are ordered by the tuple
+// (cell / B, rank, cell % B); removed particles follow in their input order.  All tuples differ,
+// so the order is unique.  Written out as the definition: S11, ranks, then a sort by the tuple.
+void orc_sort_interleaved(int64_t n, const uint32_t* cell, const uint32_t* flag, uint32_t ncells,
+                          uint32_t B, uint32_t* perm) {
+  std::vector<uint32_t> key(n), stable(n), rank(n);
+  for (int64_t k = 0; k < n; ++k) key[k] = (flag[k] & 2u) ? ncells : std::min(cell[k], ncells);
+  std::iota(stable.begin(), stable.end(), 0u);
+  std::stable_sort(stable.begin(), stable.end(), [&](uint32_t x, uint32_t y) { return key[x] < key[y]; });
+  for (int64_t k = 0, r = 0; k < n; ++k) {          // rank of the particle at sorted position k
+    r = (k > 0 && key[stable[k]] == key[stable[k - 1]]) ? r + 1 : 0;
+    rank[stable[k]] = (uint32_t)r;
+  }
+  std::copy(stable.begin(), stable.end(), perm);
+  auto before = [&](uint32_t x, uint32_t y) {
+    const bool rx = key[x] >= ncells, ry = key[y] >= ncells;
+    if (rx || ry) return !rx && ry;                  // live before removed; removed keep their order
+    if (key[x] / B != key[y] / B) return key[x] / B < key[y] / B;
+    if (rank[x] != rank[y]) return rank[x] < rank[y];
+    return key[x] % B < key[y] % B;
+  };
+  std::stable_sort(perm, perm + n, before);
 }
 
 // S12: order-preserving removal of flagged particles; idx[0..count) = surviving

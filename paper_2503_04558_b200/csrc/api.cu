@@ -185,6 +185,7 @@ int grpic_create(const grpic_params* p, grpic_ctx** out) {
   ctx->ws = nullptr;
   ctx->ws_bytes = 0;
   ctx->host_step = nullptr;
+  ctx->removed_counter = nullptr;
   cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
   GridDev& g = ctx->g;
   g.a = p->a; g.M = p->M; g.a2 = p->a * p->a; g.twoM = 2.0 * p->M;
@@ -265,9 +266,17 @@ size_t grpic_workspace_bytes(const grpic_ctx* ctx, int64_t n_particles) {
   // sort / compact: 2 key + 2 index buffers, block histograms (256 per 2048-key tile) + scan sums
   const size_t n = (size_t)n_particles;
   const size_t tiles = (n + 2047) / 2048 + 1;
+  // (+ one word per cell for the cell starts of grpic_sort_interleaved)
+  const size_t cells = (size_t)ctx->g.nr * (size_t)ctx->g.nth + 128;
   const size_t sortb = 4 * ((n + 63) & ~(size_t)63) * sizeof(uint32_t) +
-                       (256 * tiles + 4096 + tiles) * sizeof(uint32_t) * 2 + 4096;
+                       (256 * tiles + 4096 + tiles) * sizeof(uint32_t) * 2 + 4096 + cells * sizeof(uint32_t);
   return (field > sortb ? field : sortb) + 256;
+}
+
+int grpic_set_removed_counter(grpic_ctx* ctx, unsigned long long* device_counter) {
+  if (!ctx) return GRPIC_ERR_ARG;
+  ctx->removed_counter = device_counter;
+  return GRPIC_OK;
 }
 
 int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes) {

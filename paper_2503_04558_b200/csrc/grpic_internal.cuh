@@ -37,6 +37,7 @@ struct grpic_ctx {
   void* ws;
   size_t ws_bytes;
   int sm_count;
+  unsigned long long* removed_counter;   // grpic_set_removed_counter (caller's device word, nullable)
   void* host_step;  // staging buffers / streams of grpic_step_host (host_step.cu), lazily created
 };
 

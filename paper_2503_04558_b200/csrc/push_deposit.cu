@@ -175,7 +175,8 @@ __global__ void __launch_bounds__(kBlock, MINB)
 push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
                     const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
                     const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
-                    const __grid_constant__ PolyTab pt, double dt, int K, uint32_t* status) {
+                    const __grid_constant__ PolyTab pt, double dt, int K, uint32_t* status,
+                    unsigned long long* removed) {
   __shared__ WTile tiles[kWarps][kPdStages];
   __shared__ __align__(8) uint64_t full[kWarps][kPdStages];
   __shared__ uint32_t sdest[COMPACT ? kWarps : 1][kWTile];   // COMPACT: output index of each particle
@@ -404,6 +405,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     if (out) {
       nflag |= 2u;
       ncell = 0xFFFFFFFFu;
+      if (removed) atomicAdd(removed, 1ull);        // rare (a particle leaves once): lazy-removal bookkeeping
       if (status && (!finite || offgrid))
         atomicOr(status, offgrid ? GRPIC_STATUS_OFFGRID : GRPIC_STATUS_NONFINITE);
     } else {
@@ -462,7 +464,7 @@ int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const 
   const int64_t resident = (int64_t)ctx->sm_count * per_sm;
   const unsigned grid = (unsigned)(nblocks < resident ? nblocks : resident);
   push_deposit_kernel<MINB, COMPACT, KT, TAB><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, f, J, kPolyTabHost, dt,
-                                                                  ctx->p.geo_iters, status);
+                                                                  ctx->p.geo_iters, status, ctx->removed_counter);
   return grpic_launch_ok();
 }
 

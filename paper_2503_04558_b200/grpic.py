@@ -46,10 +46,10 @@ class CurrentC(C.Structure):
 
 
 EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_areas",
-           "grpic_workspace_bytes", "grpic_set_workspace", "grpic_push_deposit",
+           "grpic_workspace_bytes", "grpic_set_workspace", "grpic_set_removed_counter", "grpic_push_deposit",
            "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
-           "grpic_circulation", "grpic_sort", "grpic_compact", "grpic_deposit_rho",
+           "grpic_circulation", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_measure_fp64_issue", "grpic_kernel_launches", "grpic_strerror"]
 
 _lib = None
@@ -165,6 +165,13 @@ class Context:
             off = (-self.ws.data_ptr()) % 256
             _check(load().grpic_set_workspace(self.h, C.c_void_p(self.ws.data_ptr() + off),
                                               C.c_size_t(nbytes)))
+
+    def set_removed_counter(self, counter):
+        """counter: uint64/int64 device tensor of one element (or None): every push adds the number of
+        particles it flags removed."""
+        self._removed = counter          # keep the tensor alive while the library holds its pointer
+        ptr = C.c_void_p(counter.data_ptr()) if counter is not None else None
+        _check(load().grpic_set_removed_counter(self.h, ptr))
 
     def close(self):
         if self.h:
@@ -302,6 +309,13 @@ class Context:
         a, b = src.struct(), dst.struct()
         pp = _ptr(perm, _up) if perm is not None else None
         _check(load().grpic_sort(self.h, C.byref(a), C.byref(b), pp, _stream()))
+        dst.n = src.n
+
+    def sort_interleaved(self, src, dst, block_cells=8, perm=None):
+        self.reserve(src.n)
+        a, b = src.struct(), dst.struct()
+        pp = _ptr(perm, _up) if perm is not None else None
+        _check(load().grpic_sort_interleaved(self.h, C.byref(a), C.byref(b), pp, C.c_int32(block_cells), _stream()))
         dst.n = src.n
 
     def compact(self, src, dst, n_alive):

@@ -684,6 +684,29 @@ def test_sort_and_compact_bit_exact(G, O, n):
         assert np.all(tail["flag"][len(idx):] & 2)
 
 
+@pytest.mark.parametrize("n,B", [(0, 8), (1, 8), (33, 8), (2049, 1), (70001, 2), (70001, 8), (70001, 32), (300000, 8)])
+def test_sort_interleaved_bit_exact(G, O, n, B):
+    """grpic_sort_interleaved against the oracle's definition (S11b): permutation and reordered
+    SoA bit-exact; crowded positions (many particles per cell), empty cells, removed particles."""
+    p = inputs.grid_params(64, 48, 0.9)
+    ctx = G.Context(p, max(n, 1))
+    rng = np.random.default_rng(n + B)
+    ptc = inputs.make_particles(p, max(n, 2), 11, "crowded", ("loguniform", 0.1, 10.0))
+    ptc = {k: v[:n].copy() for k, v in ptc.items()}
+    ptc["flag"] = (ptc["flag"] | (2 * (rng.uniform(size=n) < 0.1))).astype(np.uint32)
+    src = G.Particles.from_numpy(ptc) if n else G.Particles(0)
+    dst = G.Particles(n)
+    perm = torch.zeros(max(n, 1), dtype=torch.int32, device="cuda")
+    ctx.sort_interleaved(src, dst, B, perm)
+    torch.cuda.synchronize()
+    if n:
+        pref = O.sort_interleaved(ptc["cell"], ptc["flag"], p["nr"] * p["nth"], B)
+        assert np.array_equal(perm[:n].cpu().numpy().view(np.uint32), pref)
+        got = dst.to_numpy()
+        for k in ptc:
+            assert np.array_equal(got[k], ptc[k][pref]), k
+
+
 def test_config1_ten_coupled_steps(G, O):
     """BASELINE.json config 1 at full size: 128x128, 1e5 particles, 10 x (push+deposit,
     finalize, field step N=7)."""

@@ -328,6 +328,45 @@ def test_sort_and_compact_definitions():
     assert np.array_equal(idx, np.nonzero((flag & 2) == 0)[0].astype(np.uint32))
 
 
+def test_sort_interleaved_definition():
+    """S11b: order by (cell // B, rank within the cell in stable order, cell % B), removed last in
+    input order.  Pinned by (i) a hand-built example, (ii) numpy's lexsort of the defining tuple with
+    ranks computed independently, (iii) B = 1 reducing to the plain stable sort, (iv) being a
+    permutation whose adjacent live entries of equal rank sit in different cells."""
+    # (i) cells of particles 0..7; B = 2: block 0 = cells {0,1}, block 1 = cells {2,3}
+    cell = np.array([1, 0, 1, 3, 0, 2, 1, 3], dtype=np.uint32)
+    flag = np.array([0, 0, 0, 0, 0, 2, 0, 0], dtype=np.uint32)       # particle 5 removed
+    # cell 0: particles 1,4 (ranks 0,1); cell 1: 0,2,6 (ranks 0,1,2); cell 3: 3,7 (ranks 0,1)
+    # block 0 rank-major: (r0: c0->1, c1->0), (r1: c0->4, c1->2), (r2: c1->6); block 1: 3, 7; tail: 5
+    assert list(oracle.sort_interleaved(cell, flag, 4, 2)) == [1, 0, 4, 2, 6, 3, 7, 5]
+    rng = np.random.default_rng(1)
+    n, ncells = 6000, 137
+    cell = rng.integers(0, ncells, n).astype(np.uint32)
+    flag = (rng.integers(0, 2, n) | (2 * (rng.uniform(size=n) < 0.1))).astype(np.uint32)
+    live = (flag & 2) == 0
+    for B in (1, 2, 8, 32):
+        perm = oracle.sort_interleaved(cell, flag, ncells, B)
+        assert np.array_equal(np.sort(perm), np.arange(n, dtype=np.uint32))
+        # (ii) ranks by counting earlier particles of the same cell
+        rank = np.zeros(n, dtype=np.int64)
+        seen = {}
+        for k in range(n):
+            if live[k]:
+                rank[k] = seen.get(int(cell[k]), 0)
+                seen[int(cell[k])] = rank[k] + 1
+        c = cell.astype(np.int64)
+        idx = np.arange(n)
+        order = np.lexsort((idx, np.where(live, c % B, 0), rank, np.where(live, c // B, 1 << 40)))
+        assert np.array_equal(perm, order.astype(np.uint32)), B
+        if B == 1:      # (iii)
+            assert np.array_equal(perm, oracle.sort(cell, flag))
+        # (iv) inside a block, neighbours of equal rank are in different cells
+        pc, pr = c[perm], rank[perm]
+        nl = int(live.sum())
+        same = (pc[1:nl] == pc[:nl - 1]) & (pr[1:nl] == pr[:nl - 1])
+        assert not same.any()
+
+
 # ------------------------------------------------------------------ third-order spline shape (PAPER.md:228)
 def test_spline3_shape_is_the_cubic_bspline():
     """partition of unity, first moment, variance 1/3 (cubic B-spline = 4-fold convolution of the
