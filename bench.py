@@ -36,22 +36,89 @@ if ROOT not in sys.path:
 METRIC = "GR particle push+deposit steps/sec (FP64)"
 UNIT = "particle-steps/s"
 
-# Algorithmic work of the fused push+deposit kernel per particle-step (DESIGN.md "Roofline
-# arithmetic"): FP64 pipe instructions of the method as stated (S4/S5 of SURVEY 8(c)) and
-# compulsory HBM bytes (particle state in + out; grid traffic amortised when sorted).
-# FP64: the warp-level FP64-pipe instructions (DFMA/DMUL/DADD/DSETP) the kernel EXECUTES per
-# particle, counted on ncu's source page (profiles/r01i): 623 (689 at r01c, 647 at r01f).
-# An operation count of the method as the paper states it is higher (~1190-1350); the
-# executed count is used so that `frac` equals the FP64 pipe utilisation ncu reports and is never
-# flattered by it.
-FP64_INSTR_PER_PARTICLE = 623.0
+# Work of the fused push+deposit kernel per particle-step.
+# FP64: the warp-level FP64-pipe instructions (DFMA/DMUL/DADD/DSETP) the kernel EXECUTES per particle,
+# counted on the source page of an `ncu --set full --import-source on` capture of the committed code and
+# stored, with the hash of the kernel sources it was taken on, in profiles/roofline_constants.json
+# (written by `python bench.py --ncu-constants <source-page csv> <raw-page csv>`).  An operation count of
+# the method as the paper states it is higher (~1190-1350); the executed count is used so
+# that `frac` equals the FP64 pipe utilisation ncu reports and is never flattered by it.  If the kernel
+# sources changed since the capture the roofline carries "stale": true.
 HBM_BYTES_PER_PARTICLE = 119.0
-# dram__bytes_read.sum + dram__bytes_write.sum of push_deposit_kernel<.,COMPACT> per live particle,
-# from the one `ncu --set full` capture of profiles/r01i (6.79 GB + 6.70 GB for 99.8e6 particles)
-NCU_DRAM_BYTES_PER_PARTICLE = 135.2
-# serialised-issue model (profiles/r01e, r01i): per particle 623 FP64 instructions at 2 cycles, 137 of
-# them three-register DFMAs (+1 cycle each), 585 other instructions at 1 cycle, per scheduler
-ISSUE_CYCLES_PER_PARTICLE = 623 * 2 + 137 + 585
+KERNEL_SOURCES = ("push_deposit.cu", "push_math.cuh", "poly_tables.cuh", "grpic_internal.cuh")
+CONSTANTS_FILE = os.path.join(ROOT, "profiles", "roofline_constants.json")
+
+
+def kernel_source_hash():
+    import hashlib
+    h = hashlib.sha256()
+    for f in KERNEL_SOURCES:
+        with open(os.path.join(ROOT, "paper_2503_04558_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def roofline_constants():
+    with open(CONSTANTS_FILE) as fh:
+        c = json.load(fh)
+    c["stale"] = c.get("source_hash") != kernel_source_hash()
+    return c
+
+
+def ncu_constants(source_csv, raw_csv):
+    """profiles/roofline_constants.json from the two CSV pages of one ncu capture of the push kernel:
+    `ncu -i X.ncu-rep --page source --csv` (per-instruction executed counts) and `--page raw --csv`."""
+    import csv
+    import re
+    rows = list(csv.reader(open(source_csv)))
+    kernel = rows[0][1] if len(rows[0]) > 1 else ""
+    hdr = rows[1]
+    isrc, iex = hdr.index("Source"), hdr.index("Instructions Executed")
+    fp64 = dfma3 = total = 0
+    ops = {}
+    for r in rows[2:]:
+        if len(r) <= iex:
+            continue
+        t = re.sub(r"^@!?U?P\d+\s+", "", r[isrc].strip())
+        op = t.split()[0].rstrip(";")
+        ex = int(r[iex])
+        total += ex
+        base = op.split(".")[0]
+        ops[base] = ops.get(base, 0) + ex
+        if base in ("DFMA", "DMUL", "DADD", "DSETP"):
+            fp64 += ex
+            if base == "DFMA":
+                regs = {m for o in t[len(op):].split(",")[1:] for m in re.findall(r"(?<![U])R(\d+)", o)}
+                dfma3 += ex if len(regs) >= 3 else 0
+    raw = list(csv.reader(open(raw_csv)))
+    h, v = raw[0], raw[2]
+    get = lambda name: float(v[h.index(name)].replace(",", ""))
+    unit = lambda name: raw[1][h.index(name)]
+    scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+    dram = sum(get(m) * scale[unit(m)] for m in ("dram__bytes_read.sum", "dram__bytes_write.sum"))
+    red = get("l1tex__t_requests_pipe_lsu_mem_global_op_red.sum")
+    # particles = warp-level executions of the first FP64 instruction of the push body x 32 is not exact
+    # (partial warps); the exact count is the number of STG of x1 per lane: use thread-level counts
+    ith = hdr.index("Thread Instructions Executed")
+    particles = max(int(r[ith]) for r in rows[2:] if len(r) > ith and "STG.E.EF.64" in r[isrc])
+    warps = particles / 32.0
+    out = {"source_hash": kernel_source_hash(), "kernel": kernel, "particles_in_capture": particles,
+           "fp64_instr_per_particle": fp64 / warps, "dfma_three_register_per_particle": dfma3 / warps,
+           "other_instr_per_particle": (total - fp64) / warps, "instr_per_particle": total / warps,
+           "dram_bytes_per_particle": dram / particles, "red_instr_per_particle": red / warps,
+           "duration_ms": get("gpu__time_duration.sum") * {"ms": 1.0, "us": 1e-3, "s": 1e3}[unit("gpu__time_duration.sum")],
+           "sm__pipe_fp64_cycles_active_pct": get("sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"),
+           "smsp__issue_active_pct": get("smsp__issue_active.avg.pct_of_peak_sustained_active"),
+           "registers": int(get("launch__registers_per_thread")),
+           "opcodes_per_particle": {k: round(x / warps, 2) for k, x in sorted(ops.items(), key=lambda kv: -kv[1]) if x / warps >= 0.5},
+           "how": "ncu --set full --clock-control none --import-source on -k regex:push_deposit_kernel; "
+                  "python bench.py --ncu-constants <source page csv> <raw page csv>"}
+    with open(CONSTANTS_FILE, "w") as fh:
+        json.dump(out, fh, indent=1)
+        fh.write("\n")
+    print(json.dumps(out))
+
+
 # nominal FP64 pipe: 148 SMs x 64 DFMA lanes/clk x 1.965 GHz (B200; DESIGN.md)
 FP64_NOMINAL_INSTR_PER_S = 148 * 64 * 1.965e9
 
@@ -281,8 +348,6 @@ def run_ours(args):
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         ms_total = float(t.item())
     clocks = ClockSampler.summarise(sampler.window(tw0, tw1)) if sampler else None
-    if sampler:
-        sampler.stop()
 
     # particles actually pushed per timed step (alive at the start of the step)
     if lazy:
@@ -313,9 +378,23 @@ def run_ours(args):
 
     # ---- sustained FP64 pipe rate (same clocks regime as the long step), then rooflines
     fp64_peak_sust = fp64_peak_burst
-    t_end = time.time() + 1.0
+    tp0 = time.time()
+    t_end = tp0 + 1.0
     while time.time() < t_end:
         fp64_peak_sust = ctx.measure_fp64_peak()
+    tp1 = time.time()
+    probe_clocks = ClockSampler.summarise(sampler.window(tp0 + 0.5, tp1)) if sampler else None
+    if sampler:
+        sampler.stop()
+    # The register-only DFMA probe draws less power than the step (HBM + L2 atomics + FP64): under the
+    # board's power cap the timed loop can run at a lower SM clock than the probe.  The pipe's rate is
+    # lanes x clock, so the roof the loop is held against is the probe's rate scaled to the loop's clock;
+    # the unscaled figure is reported beside it.
+    fp64_peak_probe = fp64_peak_sust
+    c_loop = (clocks or {}).get("sm_mhz")
+    c_probe = (probe_clocks or {}).get("sm_mhz")
+    if c_loop and c_probe and c_loop < c_probe:
+        fp64_peak_sust = fp64_peak_probe * c_loop / c_probe
     peaks = {}
     try:
         with open(os.path.join(ROOT, "MEASURED_PEAKS.json")) as fh:
@@ -326,32 +405,45 @@ def run_ours(args):
     hbm_src = "measured (MEASURED_PEAKS.json)" if "hbm_gbs" in peaks else "fallback"
     pd_ms = phases["push_deposit"]["ms_per_call"]
     per_launch = float(np.mean(pushed))
-    fp64_ach = FP64_INSTR_PER_PARTICLE * per_launch / (pd_ms * 1e-3)
+    rc = roofline_constants()
+    fp64_pp = float(rc["fp64_instr_per_particle"])
+    # the constants belong to one instantiation (K = 3 correctors, first-order shape, fine-grid TAB path)
+    applies = p["geo_iters"] == 3 and policy != "separate" and \
+        (("1, 3" in rc["kernel"] or "true, (int)3" in rc["kernel"]) == fused or "kernel" not in rc)
+    fp64_ach = fp64_pp * per_launch / (pd_ms * 1e-3)
     hbm_ach = HBM_BYTES_PER_PARTICLE * per_launch / (pd_ms * 1e-3) / 1e9
-    t_alu = FP64_INSTR_PER_PARTICLE * per_launch / fp64_peak_sust
+    t_alu = fp64_pp * per_launch / fp64_peak_sust
     t_hbm = HBM_BYTES_PER_PARTICLE * per_launch / (hbm_peak * 1e9)
     roofline = {
         "kernel": "push_deposit_kernel", "bound": "alu" if t_alu >= t_hbm else "hbm",
         "achieved": 2.0 * fp64_ach / 1e12, "peak": 2.0 * fp64_peak_sust / 1e12, "unit": "TFLOP/s",
         "frac": max(t_alu, t_hbm) / (pd_ms * 1e-3),
-        "traffic": NCU_DRAM_BYTES_PER_PARTICLE * per_launch,
-        "traffic_source": "ncu --set full capture of profiles/r01i (bytes per particle) x particles per launch",
-        "peak_source": "FP64 DFMA chain measured live on this device after the timed loop "
-                       "(sustained clocks); 2 flop per FP64 pipe instruction",
+        "traffic": float(rc["dram_bytes_per_particle"]) * per_launch,
+        "traffic_measured": False,
+        "traffic_source": "dram__bytes_read + write per particle of the ncu --set full capture recorded in "
+                          "profiles/roofline_constants.json x particles per launch (a constant, not this run)",
+        "constants": {"file": "profiles/roofline_constants.json", "kernel": rc.get("kernel"),
+                      "source_hash": rc.get("source_hash"), "stale": bool(rc["stale"]),
+                      "applies_to_this_run": bool(applies)},
+        "stale": bool(rc["stale"]) or not applies,
+        "peak_source": "FP64 DFMA chain measured live on this device after the timed loop, scaled to the "
+                       "SM clock sampled during the timed loop when the power cap held it below the "
+                       "probe's clock; 2 flop per FP64 pipe instruction",
+        "peak_probe": 2.0 * fp64_peak_probe / 1e12, "sm_mhz_loop": c_loop, "sm_mhz_probe": c_probe,
+        "frac_at_probe_clock": fp64_pp * per_launch / fp64_peak_probe / (pd_ms * 1e-3),
         "peak_burst": 2.0 * fp64_peak_burst / 1e12,
         "peak_nominal": 2.0 * FP64_NOMINAL_INSTR_PER_S / 1e12,
-        "fp64_instr_per_particle": FP64_INSTR_PER_PARTICLE,
+        "fp64_instr_per_particle": fp64_pp,
         "hbm": {"achieved": hbm_ach, "peak": hbm_peak, "unit": "GB/s", "frac": hbm_ach / hbm_peak,
                 "bytes_per_particle": HBM_BYTES_PER_PARTICLE, "peak_source": hbm_src},
         "launch_ms": pd_ms, "particles_per_launch": per_launch,
-        # grpic_measure_fp64_issue: cycles per warp FP64 instruction per scheduler
-        "issue_model_cycles": dict(zip(("dfma_2reg", "dfma_3reg", "dmul", "dmul_plus_3_int"),
-                                       ctx.measure_fp64_issue())),
     }
-    # the same launch against the serialised-issue bound: warps per scheduler x cycles per warp
+    # the same launch against the serialised-issue bound of its instruction mix (profiles/r01e: an FP64
+    # instruction holds the issue port 2 cycles, 3 with three register operands, any other 1 cycle)
     sm_hz = 1e6 * ((clocks or {}).get("sm_mhz") or 1965.0)
-    t_issue = ISSUE_CYCLES_PER_PARTICLE * (per_launch / 32.0) / (148 * 4) / sm_hz
-    roofline["issue_model"] = {"cycles_per_particle": ISSUE_CYCLES_PER_PARTICLE, "bound_ms": 1e3 * t_issue,
+    issue_cycles = 2.0 * fp64_pp + float(rc["dfma_three_register_per_particle"]) + float(rc["other_instr_per_particle"])
+    t_issue = issue_cycles * (per_launch / 32.0) / (148 * 4) / sm_hz
+    roofline["issue_model"] = {"cycles_per_particle": issue_cycles, "bound_ms": 1e3 * t_issue,
                                "frac": t_issue / (pd_ms * 1e-3), "sm_mhz": sm_hz / 1e6}
     # field step: cell-updates/s and HBM fraction (192 B per cell-sweep, N+1 sweeps)
     kernels = {}
@@ -618,6 +710,8 @@ def relaunch_argv(argv, gpus, port=None):
 
 def main(argv=None):
     argv = sys.argv[1:] if argv is None else argv
+    if argv and argv[0] == "--ncu-constants":
+        return ncu_constants(argv[1], argv[2])
     a = parse(argv)
     if a.impl == "reference":
         return run_reference(a)

@@ -244,13 +244,6 @@ int grpic_deposit_rho(grpic_ctx* ctx, const grpic_particles* ptc, double* rho, i
  * FP64 instructions (lane-operations) per second to the HOST double *dfma_per_second. */
 int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second);
 
-/* Issue-model probes behind the roofline discussion in DESIGN.md / profiles (blocking, ~1 ms):
- * writes to the HOST array cycles_per_instr[4] the measured cycles per warp-wide FP64
- * instruction per scheduler for  [0] DFMA with at most two register operands, [1] DFMA with three
- * distinct register operands, [2] DMUL register-register, [3] DMUL interleaved with three
- * independent integer instructions each (the excess over [2] is what the integer issue adds). */
-int grpic_measure_fp64_issue(grpic_ctx* ctx, double* cycles_per_instr);
-
 /* Number of CUDA kernels this library has launched in this process so far (all contexts);
  * used by bench.py to report `gpu_launches`. */
 int64_t grpic_kernel_launches(void);

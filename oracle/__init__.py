@@ -315,5 +315,11 @@ def shape(x):
     return float(lib().orc_shape(C.c_double(x)))
 
 
+def set_num_threads(n):
+    """OpenMP threads of the oracle's parallel loops; returns the previous setting."""
+    lib().orc_set_num_threads.restype = C.c_int
+    return int(lib().orc_set_num_threads(C.c_int(int(n))))
+
+
 def num_threads():
     return lib().orc_num_threads()

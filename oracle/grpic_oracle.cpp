@@ -215,6 +215,9 @@ void compute_areas(const Grid& g, double* ADr, double* ADth, double* ADph, doubl
                    double* ABth, double* ABph) {
   GL10 q;
   for (size_t k = 0; k < g.size(); ++k) ADr[k] = ADth[k] = ADph[k] = ABr[k] = ABth[k] = ABph[k] = 0.0;
+  // rows are independent (every iteration writes only its own node): the OpenMP loop over rows is
+  // bit-identical to the serial one (tests/test_oracle_grid.py::test_field_step_threads_bit_identical)
+#pragma omp parallel for schedule(static)
   for (int j = 0; j <= g.nth; ++j)
     for (int i = -g.G; i <= g.nr + g.G; ++i) {
       const size_t k = g.idx(i, j);
@@ -445,6 +448,7 @@ void circulation(const Grid& g, const double* ADr, const double* ADth, const dou
   const size_t n = g.size();
   std::vector<double> Hr(n, 0.0), Hth(n, 0.0), Hph(n, 0.0), Er(n, 0.0), Eth(n, 0.0), Eph(n, 0.0);
   const int ilo = -g.G + 1, ihi = g.nr + g.G - 1;  // where both i-1 and i+1 are stored
+#pragma omp parallel for schedule(static)          // row-parallel, no reduction: bit-identical to serial
   for (int j = 0; j <= g.nth; ++j)
     for (int i = ilo; i <= ihi; ++i) {
       const size_t k = g.idx(i, j);
@@ -481,6 +485,7 @@ void circulation(const Grid& g, const double* ADr, const double* ADth, const dou
                       coef(g, i - 0.5, j + 0.5).sg_beta * Bph[g.idx(i - 1, j)]);
     }
   for (size_t k = 0; k < n; ++k) CHr[k] = CHth[k] = CHph[k] = CEr[k] = CEth[k] = CEph[k] = 0.0;
+#pragma omp parallel for schedule(static)
   for (int j = 0; j <= g.nth; ++j)
     for (int i = 0; i <= g.nr; ++i) {
       const size_t k = g.idx(i, j);
@@ -1021,7 +1026,7 @@ double orc_uniform(uint64_t seed, uint32_t step, uint64_t index) {
 //    The photon's slot becomes the electron, the positron is a new particle;
 //  * new particles (photons, positrons) inherit position, cell and weight and are appended at
 //    n, n+1, ... in the order of their parents (P4).  Returns the new count (<= capacity;
-//    children beyond capacity are dropped and *overflow is set).
+//    events whose child would not fit do not happen (P5) and *overflow is set).
 int64_t orc_pair_production(const orc_params* p, int64_t n, int64_t capacity, double* x1, double* x2,
                             double* x3, double* u1, double* u2, double* u3, double* w, uint32_t* cell,
                             uint32_t* flag, double gamma_thr, double eps_ph, double p_convert,
@@ -1051,14 +1056,14 @@ int64_t orc_pair_production(const orc_params* p, int64_t n, int64_t capacity, do
       }
     }
     if (child_scale == 0.0) continue;
-    if (m < capacity) {
-      x1[m] = x1[k]; x2[m] = x2[k]; x3[m] = x3[k];
-      u1[m] = u[0] * child_scale; u2[m] = u[1] * child_scale; u3[m] = u[2] * child_scale;
-      w[m] = w[k]; cell[m] = cell[k]; flag[m] = child_flag;
-      ++m;
-    } else {
-      *overflow = 1;
+    if (m >= capacity) {                               // P5: an event whose child has no room does not
+      *overflow = 1;                                   // happen (the parent keeps momentum and species:
+      continue;                                        // no charge or momentum is lost silently)
     }
+    x1[m] = x1[k]; x2[m] = x2[k]; x3[m] = x3[k];
+    u1[m] = u[0] * child_scale; u2[m] = u[1] * child_scale; u3[m] = u[2] * child_scale;
+    w[m] = w[k]; cell[m] = cell[k]; flag[m] = child_flag;
+    ++m;
     u1[k] = u[0] * parent_scale; u2[k] = u[1] * parent_scale; u3[k] = u[2] * parent_scale;
     flag[k] = parent_flag;
   }
@@ -1071,6 +1076,19 @@ int orc_set_shape_order(int order) {
   const int old = g_shape_order;
   if (order == 1 || order == 3) g_shape_order = order;
   return old;
+}
+
+// number of OpenMP threads of the parallel loops (particles in orc_push; grid rows in the areas
+// and circulations); returns the previous value.  Used by the bit-identity test and the baseline.
+int orc_set_num_threads(int n) {
+#ifdef _OPENMP
+  const int old = omp_get_max_threads();
+  if (n > 0) omp_set_num_threads(n);
+  return old;
+#else
+  (void)n;
+  return 1;
+#endif
 }
 
 int orc_num_threads() {

@@ -119,42 +119,6 @@ __global__ void __launch_bounds__(256) dfma_kernel(double* out, int iters, doubl
   if (s == 123.456) out[0] = s;   // never true; keeps the chains alive
 }
 
-// Issue-model probes (profiles/r01c, r01e): one CTA of 1024 threads (8 warps per scheduler), eight
-// independent chains per thread, cycles per warp instruction per scheduler by clock64().
-//   KIND 0: x = fma(x, m, b), m and b loop invariants    -> 2.0 (the 64 FP64 lanes per SM)
-//   KIND 1: x = fma(y, z, x), three distinct registers    -> 3.0 (operand delivery)
-//   KIND 2: x = x * y                                     -> 2.0
-//   KIND 3: KIND 2 interleaved with 3 integer ops per DMUL -> ~2 + 3 x 0.85: the FP64 dispatch
-//           cycles are not overlapped by other issue
-template <int KIND>
-__global__ void __launch_bounds__(1024) issue_probe_kernel(double* buf, int* ibuf, long long* cyc, int n, int im) {
-  double x[8], y[8], z[8];
-  int a[8];
-  for (int k = 0; k < 8; ++k) {
-    x[k] = buf[threadIdx.x] + k; y[k] = buf[threadIdx.x + 1] + 0.5 * k; z[k] = buf[threadIdx.x + 2] - k;
-    a[k] = threadIdx.x + k;
-  }
-  const double m = 0.999999, b = 1e-9;
-  __syncthreads();
-  const long long t0 = clock64();
-  for (int i = 0; i < n; ++i) {
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      if (KIND == 0) x[k] = fma(x[k], m, b);
-      if (KIND == 1) x[k] = fma(y[k], z[k], x[k]);
-      if (KIND >= 2) x[k] = x[k] * y[k];
-      if (KIND == 3) a[k] = (a[k] ^ im) + (a[(k + 1) & 7] & 0x55);
-    }
-  }
-  const long long t1 = clock64();
-  double s = 0.0;
-  int t = 0;
-  for (int k = 0; k < 8; ++k) { s += x[k]; t += a[k]; }
-  buf[threadIdx.x] = s * 1e-300;
-  ibuf[threadIdx.x] = t;
-  if (threadIdx.x == 0) cyc[0] = t1 - t0;
-}
-
 int launch_areas(const GridDev& g, double* const out[6], int factors, cudaStream_t st) {
   dim3 block(128), grid((g.pitch + 127) / 128, g.rows);
   areas_kernel<<<grid, block, 0, st>>>(g, out[0], out[1], out[2], out[3], out[4], out[5], factors);
@@ -308,36 +272,6 @@ int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second) {
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   *dfma_per_second = best;
-  return grpic_launch_ok();
-}
-
-int grpic_measure_fp64_issue(grpic_ctx* ctx, double* cycles_per_instr) {
-  if (!ctx || !cycles_per_instr) return GRPIC_ERR_ARG;
-  double* buf = ctx->tables;                 // scratch: the probes restore nothing they need
-  double keep[1032];
-  int* ibuf = nullptr;
-  long long* cyc = nullptr;
-  GRPIC_CUDA_OK(cudaMemcpy(keep, buf, sizeof(keep), cudaMemcpyDeviceToHost));
-  if (cudaMalloc(&ibuf, 1024 * sizeof(int) + 64) != cudaSuccess) return GRPIC_ERR_ALLOC;
-  cyc = (long long*)(ibuf + 1024);
-  const int n = 2000;
-  long long h[4] = {0, 0, 0, 0};
-  for (int kind = 0; kind < 4; ++kind) {
-    GRPIC_CUDA_OK(cudaMemset(buf, 0, sizeof(keep)));
-    if (kind == 0) issue_probe_kernel<0><<<1, 1024>>>(buf, ibuf, cyc, n, 3);
-    if (kind == 1) issue_probe_kernel<1><<<1, 1024>>>(buf, ibuf, cyc, n, 3);
-    if (kind == 2) issue_probe_kernel<2><<<1, 1024>>>(buf, ibuf, cyc, n, 3);
-    if (kind == 3) issue_probe_kernel<3><<<1, 1024>>>(buf, ibuf, cyc, n, 3);
-    if (cudaMemcpy(&h[kind], cyc, sizeof(long long), cudaMemcpyDeviceToHost) != cudaSuccess) {
-      cudaFree(ibuf);
-      return GRPIC_ERR_CUDA;
-    }
-  }
-  grpic_count_launches(4);
-  cudaMemcpy(buf, keep, sizeof(keep), cudaMemcpyHostToDevice);
-  cudaFree(ibuf);
-  // 8 warps per scheduler, 8 FP64 instructions per thread per iteration
-  for (int kind = 0; kind < 4; ++kind) cycles_per_instr[kind] = (double)h[kind] / (double)n / 8.0 / 8.0;
   return grpic_launch_ok();
 }
 

@@ -127,6 +127,13 @@ extern "C" int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_
   for (int c = 0; c < 3; ++c) GRPIC_CUDA_OK(cudaMemsetAsync(S->flux[c], 0, n2 * sizeof(double), st));
   GRPIC_CUDA_OK(cudaMemsetAsync(S->status_dev, 0, sizeof(uint32_t), st));
 
+  // an error return must not leave copies into the caller's host memory in flight
+  auto fail = [&](int code) -> int {
+    cudaStreamSynchronize(S->s_h2d);
+    cudaStreamSynchronize(S->s_d2h);
+    cudaStreamSynchronize(st);
+    return code;
+  };
   const int64_t nchunks = (n + chunk - 1) / chunk;
   int64_t written = 0;                                // survivors copied back so far
   auto finish = [&](int64_t c) -> int {               // chunk c: count known -> copy survivors home
@@ -146,7 +153,7 @@ extern "C" int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_
     // input buffer b is free once the push of chunk c-2 has read it
     if (c >= kBufs) GRPIC_CUDA_OK(cudaStreamWaitEvent(S->s_h2d, S->push_done[b], 0));
     rc = copy_soa(S->in[b], 0, *host_ptc, lo, m, false, cudaMemcpyHostToDevice, S->s_h2d);
-    if (rc != GRPIC_OK) return rc;
+    if (rc != GRPIC_OK) return fail(rc);
     GRPIC_CUDA_OK(cudaEventRecord(S->h2d_done[b], S->s_h2d));
     GRPIC_CUDA_OK(cudaStreamWaitEvent(st, S->h2d_done[b], 0));
     if (c >= kBufs) GRPIC_CUDA_OK(cudaStreamWaitEvent(st, S->d2h_done[b], 0));   // output buffer b drained
@@ -154,19 +161,19 @@ extern "C" int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_
     in.n = m;
     out.n = m;
     rc = grpic_push_deposit_compact(ctx, &in, &out, fields, &flux, dt, S->n_alive_dev + b, S->status_dev, st);
-    if (rc != GRPIC_OK) return rc;
+    if (rc != GRPIC_OK) return fail(rc);
     GRPIC_CUDA_OK(cudaMemcpyAsync(S->n_alive_pin + b, S->n_alive_dev + b, sizeof(int64_t),
                                   cudaMemcpyDeviceToHost, st));
     GRPIC_CUDA_OK(cudaEventRecord(S->push_done[b], st));
-    if (c >= 1) { rc = finish(c - 1); if (rc != GRPIC_OK) return rc; }
+    if (c >= 1) { rc = finish(c - 1); if (rc != GRPIC_OK) return fail(rc); }
   }
-  if (nchunks >= 1) { rc = finish(nchunks - 1); if (rc != GRPIC_OK) return rc; }
+  if (nchunks >= 1) { rc = finish(nchunks - 1); if (rc != GRPIC_OK) return fail(rc); }
 
   // grid part of the step on the caller's stream, overlapping the last copies home
   rc = grpic_finalize_current(ctx, &flux, filter_passes, st);
-  if (rc != GRPIC_OK) return rc;
+  if (rc != GRPIC_OK) return fail(rc);
   rc = grpic_field_step(ctx, fields, &flux, background, dt, st);
-  if (rc != GRPIC_OK) return rc;
+  if (rc != GRPIC_OK) return fail(rc);
   if (host_J) {
     double* const hj[3] = {host_J->Fr, host_J->Fth, host_J->Fph};
     for (int c = 0; c < 3; ++c)

@@ -103,11 +103,10 @@ pair_apply_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grp
   if (!child) return;
   const double ur = P.u1[k], ut = P.u2[k], up = P.u3[k];
   const int64_t d = P.n + (int64_t)offsets[tile] + __popc(b & ((1u << lane) - 1u));
-  if (d < capacity) {
-    P.x1[d] = P.x1[k]; P.x2[d] = P.x2[k]; P.x3[d] = P.x3[k];
-    P.u1[d] = ur * e.child_scale; P.u2[d] = ut * e.child_scale; P.u3[d] = up * e.child_scale;
-    P.w[d] = P.w[k]; P.cell[d] = P.cell[k]; P.flag[d] = e.child_flag;
-  }
+  if (d >= capacity) return;      // P5: an event whose child has no room does not happen (parent unchanged)
+  P.x1[d] = P.x1[k]; P.x2[d] = P.x2[k]; P.x3[d] = P.x3[k];
+  P.u1[d] = ur * e.child_scale; P.u2[d] = ut * e.child_scale; P.u3[d] = up * e.child_scale;
+  P.w[d] = P.w[k]; P.cell[d] = P.cell[k]; P.flag[d] = e.child_flag;
   P.u1[k] = ur * e.parent_scale; P.u2[k] = ut * e.parent_scale; P.u3[k] = up * e.parent_scale;
   P.flag[k] = e.parent_flag;
 }

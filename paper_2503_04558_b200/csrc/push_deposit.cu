@@ -150,8 +150,7 @@ constexpr int kWTile = 64;
 constexpr int kPdStages = GRPIC_PD_STAGES;   // particle tiles in flight per warp
 struct __align__(128) WTile {
   double x1[kWTile], x2[kWTile], x3[kWTile], u1[kWTile], u2[kWTile], u3[kWTile], w[kWTile];
-  uint32_t flag[kWTile];
-  uint32_t ob[4];   // COMPACT: the aligned 16 bytes of `offsets` that hold this tile's two output offsets
+  uint32_t flag[kWTile];   // bits 0-2: species / removed; COMPACT parks the lane's output rank in bits 8-13
 };
 constexpr uint32_t kTileBytes = 7u * kWTile * 8u + kWTile * 4u;
 
@@ -179,7 +178,10 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
                     unsigned long long* removed) {
   __shared__ WTile tiles[kWarps][kPdStages];
   __shared__ __align__(8) uint64_t full[kWarps][kPdStages];
-  __shared__ uint32_t sdest[COMPACT ? kWarps : 1][kWTile];   // COMPACT: output index of each particle
+  // COMPACT: the aligned 16 bytes of `offsets` that hold each staged tile's two output offsets.
+  // Shared memory is kept below 15872 bytes per CTA on purpose: 8 CTAs then fit the 132 KB carve-out
+  // and leave 124 KB of L1 to the gather (the 164 KB carve-out a few bytes more would select: 92 KB).
+  __shared__ __align__(16) uint32_t sob[COMPACT ? kWarps : 1][COMPACT ? kPdStages : 1][4];
   uint32_t tid_x;
   asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
   const uint32_t lane = tid_x & 31u;
@@ -202,7 +204,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       uint64_t* bar = &bars[stage];
       mbar_expect_tx(bar, kTileBytes + (COMPACT ? 16u : 0u));
       // the tile's two output offsets ride along (offsets[2 tile], [2 tile + 1], inside an aligned 16 bytes)
-      if (COMPACT) tma_load_1d(T.ob, offsets + ((2u * tile) & ~3u), 16, bar, stream_policy);
+      if (COMPACT) tma_load_1d(sob[warp][stage], offsets + ((2u * tile) & ~3u), 16, bar, stream_policy);
       tma_load_1d(T.x1, ptc.x1 + k0, kWTile * 8, bar, stream_policy);
       tma_load_1d(T.x2, ptc.x2 + k0, kWTile * 8, bar, stream_policy);
       tma_load_1d(T.x3, ptc.x3 + k0, kWTile * 8, bar, stream_policy);
@@ -244,24 +246,26 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
           T.flag[s2] = 2u;
         }
       }
-      if (COMPACT && lane < 4) T.ob[lane] = offsets[((2u * tile) & ~3u) + lane];
+      if (COMPACT && lane < 4) sob[warp][stage][lane] = offsets[((2u * tile) & ~3u) + lane];
       __syncwarp();
     }
     if (COMPACT) {
-      // rank of each particle among the live lanes of its 32-particle half, parked in shared
-      // memory instead of registers that would live across the whole push
+      // rank of each particle among the live lanes of its 32-particle half, parked in the spare bits
+      // of its flag word in shared memory instead of a register that would live across the whole push
       uint32_t lt;
       asm("mov.u32 %0, %%lanemask_lt;" : "=r"(lt));
-      const uint32_t live0 = __ballot_sync(0xffffffffu, !(T.flag[lane] & 2u));
-      const uint32_t live1 = __ballot_sync(0xffffffffu, !(T.flag[32 + lane] & 2u));
-      sdest[warp][lane] = __popc(live0 & lt);
-      sdest[warp][32 + lane] = __popc(live1 & lt);
+      const uint32_t f0 = T.flag[lane], f1 = T.flag[32 + lane];
+      const uint32_t live0 = __ballot_sync(0xffffffffu, !(f0 & 2u));
+      const uint32_t live1 = __ballot_sync(0xffffffffu, !(f1 & 2u));
+      T.flag[lane] = (f0 & 7u) | (__popc(live0 & lt) << 8);
+      T.flag[32 + lane] = (f1 & 7u) | (__popc(live1 & lt) << 8);
     }
   }
 
   {
   const uint32_t sl = half * 32 + lane;
-  const uint32_t flag = T.flag[sl];
+  const uint32_t flag_word = T.flag[sl];
+  const uint32_t flag = COMPACT ? (flag_word & 7u) : flag_word;
   if (!(flag & 2u)) {
     const double x1 = T.x1[sl], x2 = T.x2[sl];
     // species: charge sign of e-/e+; a photon (bit2) feels no Lorentz force
@@ -346,7 +350,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 #pragma unroll
     for (int ci = 0; ci < KK; ++ci) {
       double s, c;
-      if (fabs(dth) <= kSmallStep) sincos_shift(pt, s0, c0, dth, s, c);
+      // TAB: |dtheta| = dt |X^theta| <= dt alpha / rho <= dt / r < kSmallStep is guaranteed by the dispatch
+      if (TAB || fabs(dth) <= kSmallStep) sincos_shift(pt, s0, c0, dth, s, c);
       else sincos_pt(pt, x2 + dth, s, c);
       const Pos p1 = make_pos(g, r0 + dr, s, c);
       double Xr, Xt, Xp, Ur, Ut;
@@ -363,8 +368,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     // ---- new logical position: ln r = x1 + 2 atanh(dr / (2 r0 + dr)) ----
     double x1n;
     {
-      const double wq = dr * rcp_nr(r0 + r);
-      if (fabs(wq) <= 0.03) {
+      const double wq = dr * rcp_nr(r0 + r);       // TAB: |dr| <= dt << r, the series always applies
+      if (TAB || fabs(wq) <= 0.03) {
         const double w2 = wq * wq;
         double pl = fma(w2, pt.v[kR11], pt.v[kR9]);
         pl = fma(pl, w2, pt.v[kR7]);
@@ -420,7 +425,7 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       ncell = (uint32_t)(jc * g.nr + ic);
     }
     // COMPACT: output index = offsets[this 32-particle half] + rank among its live lanes
-    const uint32_t kd = COMPACT ? T.ob[(tile & 1u) * 2u + half] + sdest[warp][sl] : tile * kWTile + sl;
+    const uint32_t kd = COMPACT ? sob[warp][stage][(tile & 1u) * 2u + half] + (T.flag[sl] >> 8) : tile * kWTile + sl;
     __stcs(dst.x1 + kd, x1n); __stcs(dst.x2 + kd, th); __stcs(dst.x3 + kd, ph);   // streaming stores
     __stcs(dst.u1 + kd, vr); __stcs(dst.u2 + kd, vt); __stcs(dst.u3 + kd, up);
     if (COMPACT) __stcs(dst.w + kd, T.w[sl]);
@@ -472,18 +477,23 @@ template <bool COMPACT>
 int dispatch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
                           const uint32_t* offsets, const grpic_fields& f,
                           const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
-  // tuning knob (read once): GRPIC_PD_MINB=4 selects the 126-register build (GRPIC_PD_MA CTAs per
-  // SM), anything else the 96-register one (GRPIC_PD_MB); defaults: compacting -> 126, in place -> 96
+  // tuning knob (read once): GRPIC_PD_MINB = resident 64-thread CTAs per SM the kernel is built for:
+  // 8 (<= 128 registers, no spills: the default; 5.70 ms per push averaged over a 20-step sort period at
+  // 1e8 particles), 9 (<= 112: 5.90 ms) or 10 (<= 96: 5.99 ms) -- profiles/r02h
   static int minb = -1;
-  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : (COMPACT ? 4 : 5); }
-  // TAB: cells small enough for the node-table + in-cell series form of r, sin, cos (push_math.cuh)
-  const bool tab = ctx->g.dxi <= kSmallStep && ctx->g.dth <= kSmallStep;
+  if (minb < 0) { const char* e = getenv("GRPIC_PD_MINB"); minb = e ? atoi(e) : 8; }
+  // TAB: cells small enough for the node-table + in-cell series form of r, sin, cos (push_math.cuh),
+  // and a time step whose moves |dtheta| <= dt / r, |dr| <= dt stay inside the short series of the
+  // correctors and of ln r without a test (r >= r_in - dt during the iterations; factor 2 of margin)
+  const bool tab = ctx->g.dxi <= kSmallStep && ctx->g.dth <= kSmallStep && 2.0 * dt <= kSmallStep * exp(ctx->g.xi_in);
   if (ctx->p.geo_iters != 3)
     return launch_push_deposit<GRPIC_PD_MA, COMPACT, 0, false>(ctx, ptc, dst, offsets, f, J, dt, status, st);
   if (!tab)
     return launch_push_deposit<GRPIC_PD_MA, COMPACT, 3, false>(ctx, ptc, dst, offsets, f, J, dt, status, st);
-  if (minb == 4)
+  if (minb <= 8)
     return launch_push_deposit<GRPIC_PD_MA, COMPACT, 3, true>(ctx, ptc, dst, offsets, f, J, dt, status, st);
+  if (minb == 9)
+    return launch_push_deposit<9, COMPACT, 3, true>(ctx, ptc, dst, offsets, f, J, dt, status, st);
   return launch_push_deposit<GRPIC_PD_MB, COMPACT, 3, true>(ctx, ptc, dst, offsets, f, J, dt, status, st);
 }
 

@@ -50,7 +50,7 @@ EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_area
            "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
-           "grpic_measure_fp64_peak", "grpic_measure_fp64_issue", "grpic_kernel_launches", "grpic_strerror"]
+           "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
 
 _lib = None
 
@@ -331,13 +331,6 @@ class Context:
         v = C.c_double(0.0)
         _check(load().grpic_measure_fp64_peak(self.h, C.byref(v)))
         return v.value
-
-    def measure_fp64_issue(self):
-        """cycles per warp-wide FP64 instruction per scheduler: [DFMA <= 2 register operands,
-        DFMA 3 register operands, DMUL, DMUL + 3 integer instructions]"""
-        v = (C.c_double * 4)()
-        _check(load().grpic_measure_fp64_issue(self.h, v))
-        return [float(x) for x in v]
 
     @staticmethod
     def kernel_launches():

@@ -69,27 +69,53 @@ def oracle_push_deposit(O, p, fields, ptc, dt):
     return new, F
 
 
-def check_push(p, ptc, ref, got, O=None, fields=None, dt=None, tol=1e-12, max_frac=1e-4):
-    """x,u <= 1e-12 (G20 norm); integer outputs bit-exact outside the edge-ambiguous set.
-    Ill-conditioned particles (a stiff 1/sin^3 force within ~1e-3 cell of the axis amplifies
-    one ulp of the input by > 1e4) are compared at 10x the oracle's OWN sensitivity to a
-    4-ulp perturbation of the input position."""
+AXIS_BAND = 1e-3      # sin(theta) below which the comparison uses the conditioning rule
+PARITY_LOG = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out", "parity_stats.jsonl")
+
+
+def check_push(p, ptc, ref, got, O=None, fields=None, dt=None, tol=1e-12, max_over=0, label=""):
+    """DESIGN.md section 7 "comparison rule for x, u".  G20 norm per particle.
+    * Every particle with sin(theta) >= AXIS_BAND before and after the step: x, u <= 1e-12, no exception.
+    * Inside the band the geodesic force ~ u_phi^2 cos/sin^3 amplifies one ulp of the input by up to
+      1/sin^3: there the bound is max(1e-12, 10 x the oracle's OWN response to a 4-ulp change of the
+      input position), and at most `max_over` particles of the case may exceed 1e-12 at all (set per
+      call site to <= 2x the count measured on B200, printed and logged to gpurun_out/parity_stats.jsonl:
+      0 everywhere except BASELINE config 1, whose 1e5 particles are uniform in theta down to 1e-9).
+    * cell / flag bit-exact outside the edge-ambiguous set (G20)."""
+    import json
     amb = edge_ambiguous(p, ref)
     ex = ptc_err(ref, got, ("x1", "x2", "x3"))
     eu = ptc_err(ref, got, ("u1", "u2", "u3"))
-    tolk = np.full(len(ex), tol)
-    if O is not None:
+    err = np.maximum(ex, eu)
+    near_axis = (np.sin(ptc["x2"]) < AXIS_BAND) | (np.sin(np.clip(ref["x2"], 0.0, math.pi)) < AXIS_BAND)
+    tolk = np.full(len(err), tol)
+    sens = np.zeros(len(err))
+    if O is not None and near_axis.any():
         eps = 4 * np.finfo(np.float64).eps
         pert = dict(ptc)
         pert["x1"] = ptc["x1"] * (1.0 + eps)
         pert["x2"] = ptc["x2"] * (1.0 + eps)
         refp = O.push(p, fields, pert, dt)
         sens = np.maximum(ptc_err(ref, refp, ("x1", "x2", "x3")), ptc_err(ref, refp, ("u1", "u2", "u3")))
-        tolk = np.maximum(tolk, 10.0 * sens)
-    # the set that actually exceeds the plain tolerance must be tiny (it was 1 in 1e5 on config 1)
-    assert (np.maximum(ex, eu) > tol).mean() <= max_frac, (np.maximum(ex, eu) > tol).mean()
-    assert np.all(ex <= tolk), ("x", ex.max(), int(ex.argmax()))
-    assert np.all(eu <= tolk), ("u", eu.max(), int(eu.argmax()))
+        tolk = np.where(near_axis, np.maximum(tol, 10.0 * sens), tol)
+    over = err > tol
+    stats = {"case": label or os.environ.get("PYTEST_CURRENT_TEST", "").split(" ")[0], "n": int(len(err)),
+             "n_near_axis": int(near_axis.sum()), "n_over_1e-12": int(over.sum()),
+             "worst_err": float(err.max()) if len(err) else 0.0,
+             "worst_err_outside_band": float(err[~near_axis].max()) if (~near_axis).any() else 0.0,
+             "worst_err_over_sens": float((err[over] / np.maximum(sens[over], 1e-300)).max()) if over.any() else 0.0,
+             "max_sin_theta_of_over": float(np.sin(ptc["x2"][over]).max()) if over.any() else 0.0,
+             "edge_ambiguous": int(amb.sum())}
+    print("parity", json.dumps(stats))
+    try:
+        os.makedirs(os.path.dirname(PARITY_LOG), exist_ok=True)
+        with open(PARITY_LOG, "a") as fh:
+            fh.write(json.dumps(stats) + "\n")
+    except OSError:
+        pass
+    assert not (over & ~near_axis).any(), ("outside the axis band", stats)
+    assert int(over.sum()) <= max_over, stats
+    assert np.all(err <= tolk), stats
     ok = ~amb
     assert np.array_equal(ref["cell"][ok], got["cell"][ok])
     assert np.array_equal(ref["flag"][ok], got["flag"][ok])
@@ -156,7 +182,7 @@ def test_axis_crossers_and_leavers(G, O):
     assert (ref["x2dep"] < 0).sum() > 50 and (ref["x2dep"] > np.pi).sum() > 50
     assert (ref["flag"] & 2).sum() > 100
     ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
-    check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-2)
+    check_push(p, ptc, ref, P.to_numpy(), O, fields, dt)
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
     # a second step must leave the removed particles untouched and deposit nothing for them
@@ -209,7 +235,7 @@ def test_push_deposit_compact_equals_compact_then_push(G, O, n, frac):
         return
     ref, Fref = oracle_push_deposit(O, p, fields, sub, dt)
     head = {k: v[:m] for k, v in got.items()}
-    check_push(p, sub, ref, head, O, fields, dt, max_frac=1e-3)
+    check_push(p, sub, ref, head, O, fields, dt)
     assert np.array_equal(head["w"], sub["w"])
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
@@ -241,7 +267,7 @@ def test_step_host_matches_oracle_step(G, O, n, chunk):
         ref, Fref = oracle_push_deposit(O, p, fields, sub, dt)
         got = {k: host[k][:m].numpy() for k in ("x1", "x2", "x3", "u1", "u2", "u3", "w")}
         got.update({k: host[k][:m].numpy().view(np.uint32) for k in ("cell", "flag")})
-        check_push(p, sub, ref, got, O, fields, dt, max_frac=1e-3)
+        check_push(p, sub, ref, got, O, fields, dt)
         assert np.array_equal(got["w"], sub["w"])
     else:
         Fref = [np.zeros_like(fields[0]) for _ in range(3)]
@@ -265,7 +291,7 @@ def test_photon_species_parity(G, O):
     ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
     ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
     got = P.to_numpy()
-    check_push(p, ptc, ref, got, O, fields, dt, max_frac=1e-3)
+    check_push(p, ptc, ref, got, O, fields, dt)
     assert np.array_equal(got["flag"] & 4, ptc["flag"] & 4)
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
@@ -332,7 +358,7 @@ def test_far_moves_take_the_general_window(G, O):
     ctx, P, F_t = gpu_push_deposit(G, p, fields, ptc, dt)
     st = int(ctx.status.item())
     assert st & 1 and not (st & ~1)
-    check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-3)
+    check_push(p, ptc, ref, P.to_numpy(), O, fields, dt)
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
 
@@ -358,7 +384,7 @@ def test_spline3_push_deposit_parity(G, O):
     torch.cuda.synchronize()
     assert int(ctx.status.item()) == 0
     with O.shape_order(3):
-        check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-3)
+        check_push(p, ptc, ref, P.to_numpy(), O, fields, dt)
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
     ctx2 = G.Context(inputs.grid_params(48, 40, 0.99), 16)                         # ng = 2: refused
@@ -511,7 +537,7 @@ def test_push_deposit_variants_parity(G, O, order, pusher):
     torch.cuda.synchronize()
     assert int(ctx.status.item()) == 0
     with O.shape_order(order), O.pusher(pusher):
-        check_push(p, ptc, ref, P.to_numpy(), O, fields, dt, max_frac=1e-3)
+        check_push(p, ptc, ref, P.to_numpy(), O, fields, dt)
     for c in range(3):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
     if pusher == 1:     # the option matters: Vay and Boris momenta differ at O(dt^3) per step
@@ -737,7 +763,7 @@ def test_config1_ten_coupled_steps(G, O):
         ctx.field_step(f_t, F_t, dt)
         if step == 0:
             torch.cuda.synchronize()
-            check_push(p, ptc, new, P.to_numpy(), O, fields_before, dt)
+            check_push(p, ptc, new, P.to_numpy(), O, fields_before, dt, max_over=10)   # measured on B200: 5 of 1e5, all with sin(theta) < 3.6e-4
             for c in range(3):
                 assert grid_err(J[c], ctx.to_host(F_t[c])) <= 1e-11
             for c in range(6):
@@ -925,3 +951,189 @@ def test_config3_full_size_bench_path(G, O):
     dphi = got1["x3"] - ptc["x3"][perm]
     Fph = ctx.to_host(F1[2])
     assert abs(Fph.sum() - np.sum(Q * dphi) / dt) <= 1e-9 * np.sum(np.abs(Q * dphi)) / dt
+
+
+# ------------------------------------------------------------------ full-size cases added in round 2
+@pytest.mark.parametrize("N", [2048, 4096])
+def test_field_step_full_size_parity(G, O, N):
+    """One full grpic_field_step (predictor + 7 correctors, axis / guard conditions, damping over the
+    outer 10 % of the radial cells, prescribed random J) at the sizes bench.py runs: 2048^2 (configs[2],
+    [4]) and BASELINE.json configs[3]'s 4096^2, in the launch shape of those sizes (32-row chunks,
+    several waves of CTAs, TMA row rings), element by element against the oracle: <= 1e-11 of the
+    array's max.  The second field step is compared at 2048^2 too (the
+    first one's output, guards included, is the second one's input)."""
+    cfg = inputs.config(4, nr=N, nth=N)
+    p, dt = cfg["params"], cfg["dt"]
+    ctx = G.Context(p, 16)
+    f_t = [ctx.to_device(x) for x in cfg["fields"]]
+    bg_t = [ctx.to_device(x) for x in cfg["bg"]]
+    J_t = [ctx.to_device(x) for x in cfg["J"]]
+    ctx.fill_guards(f_t)
+    fo = [x.copy() for x in cfg["fields"]]
+    steps = 2 if N == 2048 else 1
+    for s in range(steps):
+        ctx.field_step(f_t, J_t, dt, bg_t)
+        O.field_step(p, fo, cfg["J"], dt, bg=cfg["bg"])
+        torch.cuda.synchronize()
+        for c in range(6):
+            got = ctx.to_host(f_t[c])
+            assert np.all(np.isfinite(got))
+            assert grid_err(fo[c], got) <= 1e-11, (N, s, c, grid_err(fo[c], got))
+
+
+def test_config3_full_size_interleaved_lazy_path(G, O):
+    """The path bench.py times by default since round 2, at BASELINE.json config 3's full size (2048^2,
+    1e8 particles): grpic_sort_interleaved (block of 8 cells) -- permutation bit-exact against the
+    oracle's definition S11b on all 1e8 particles -- then two IN-PLACE pushes with lazy removal: the
+    removed counters equal the number of flags set, flagged particles are skipped by the second
+    push (state untouched), a sample is pushed one by one by the oracle through both steps."""
+    cfg = inputs.config(3)
+    p, dt, fields, ptc = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    n = len(ptc["x1"])
+    ctx = G.Context(p, n)
+    f_t = [ctx.to_device(f) for f in fields]
+    A, B = G.Particles.from_numpy(ptc), G.Particles(n)
+    perm_t = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.sort_interleaved(A, B, 8, perm_t)
+    torch.cuda.synchronize()
+    perm = perm_t.cpu().numpy().view(np.uint32)
+    del perm_t, A
+    assert np.array_equal(perm, O.sort_interleaved(ptc["cell"], ptc["flag"], p["nr"] * p["nth"], 8))
+    removed = torch.zeros(2, dtype=torch.int64, device="cuda")
+    F1, F2 = ctx.zeros(3), ctx.zeros(3)
+    ctx.status.zero_()
+    ctx.set_removed_counter(removed[0:1])
+    ctx.push_deposit(B, f_t, F1, dt)
+    torch.cuda.synchronize()
+    got1 = B.to_numpy()
+    ctx.set_removed_counter(removed[1:2])
+    ctx.push_deposit(B, f_t, F2, dt)
+    ctx.set_removed_counter(None)
+    torch.cuda.synchronize()
+    got2 = B.to_numpy()
+    assert int(ctx.status.item()) == 0
+    gone1 = (got1["flag"] & 2) != 0
+    gone2 = (got2["flag"] & 2) != 0
+    r = removed.cpu().numpy()
+    assert int(r[0]) == int(gone1.sum()) > 0 and int(r[0] + r[1]) == int(gone2.sum())
+    for k in ("x1", "x2", "x3", "u1", "u2", "u3"):          # lazily removed particles are not touched again
+        assert np.array_equal(got2[k][gone1], got1[k][gone1]), k
+    rng = np.random.default_rng(4)
+    sample = np.union1d(np.sort(rng.choice(n, 200_000, replace=False)), np.flatnonzero(gone1)[:5000])
+    src = perm[sample]
+    sub = {k: np.ascontiguousarray(v[src]) for k, v in ptc.items()}
+    ref1 = O.push(p, fields, sub, dt)
+    check_push(p, sub, ref1, {k: got1[k][sample] for k in got1}, O, fields, dt, label="c3 lazy step 1")
+    sub2 = {k: np.ascontiguousarray(ref1[k]) for k in ("x1", "x2", "x3", "u1", "u2", "u3", "cell", "flag")}
+    sub2["w"] = sub["w"]
+    ref2 = O.push(p, fields, sub2, dt)
+    check_push(p, sub2, ref2, {k: got2[k][sample] for k in got2}, O, fields, dt, tol=1e-11,
+               label="c3 lazy step 2")
+    Q = np.where(ptc["flag"][perm] & 1, 1.0, -1.0) * ptc["w"][perm]
+    dphi = got1["x3"] - ptc["x3"][perm]
+    Fph = ctx.to_host(F1[2])
+    assert abs(Fph.sum() - np.sum(Q * dphi) / dt) <= 1e-9 * np.sum(np.abs(Q * dphi)) / dt
+
+
+def test_config2_multi_step_loop_reduced(G, O):
+    """BASELINE.json config 2's recipe ("100 steps, sort every 20 steps", fields frozen) at reduced size
+    (128^2, 60000 particles = 30000 pairs), 45 steps with a cell sort at steps 0, 20 and 40, both sort
+    orders: particle ORDER, cells and flags bit-exact against the oracle loop after every sort; the
+    float state within the accumulated-conditioning bound of section 7 at the end."""
+    cfg = inputs.config(2, nr=128, nth=128, n=30000)
+    p, dt, fields, ptc0 = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    n = len(ptc0["x1"])
+    ncells = p["nr"] * p["nth"]
+    for order in ("stable", "interleaved"):
+        ctx = G.Context(p, n)
+        f_t = [ctx.to_device(f) for f in fields]
+        A, B = G.Particles.from_numpy(ptc0), G.Particles(n)
+        cur = {k: v.copy() for k, v in ptc0.items()}
+        eps = 4 * np.finfo(np.float64).eps
+        cur2 = dict(cur, x1=cur["x1"] * (1 + eps), x2=cur["x2"] * (1 + eps))
+        F_t = ctx.zeros(3)
+        for step in range(45):
+            if step % 20 == 0:
+                perm = O.sort(cur["cell"], cur["flag"]) if order == "stable" else \
+                    O.sort_interleaved(cur["cell"], cur["flag"], ncells, 8)
+                cur = {k: np.ascontiguousarray(v[perm]) for k, v in cur.items()}
+                cur2 = {k: np.ascontiguousarray(v[perm]) for k, v in cur2.items()}
+                if order == "stable":
+                    ctx.sort(A, B)
+                else:
+                    ctx.sort_interleaved(A, B, 8)
+                A, B = B, A
+                torch.cuda.synchronize()
+                got = A.to_numpy()
+                same = got["flag"] == cur["flag"]
+                # the order is decided by integer keys: identical as long as the cells agree
+                assert np.array_equal(got["cell"], cur["cell"]) and same.all(), (order, step)
+                assert np.array_equal(got["w"], cur["w"])
+            new = O.push(p, fields, cur, dt)
+            new2 = O.push(p, fields, cur2, dt)
+            for k in ("x1", "x2", "x3", "u1", "u2", "u3", "cell", "flag"):
+                cur[k], cur2[k] = new[k], new2[k]
+            ctx.push_deposit(A, f_t, F_t, dt)
+        torch.cuda.synchronize()
+        got = A.to_numpy()
+        ok = (got["flag"] == cur["flag"]) & (cur2["flag"] == cur["flag"])
+        assert ok.mean() > 0.9999
+        sens = np.maximum(ptc_err(cur, cur2, ("x1", "x2", "x3")), ptc_err(cur, cur2, ("u1", "u2", "u3")))
+        err = np.maximum(ptc_err(cur, got, ("x1", "x2", "x3")), ptc_err(cur, got, ("u1", "u2", "u3")))
+        print("parity c2 loop", order, "worst", err[ok].max(), "over 1e-10:", int((err[ok] > 1e-10).sum()))
+        assert np.all(err[ok] <= np.maximum(1e-10, 100.0 * sens[ok]))
+        assert (err[ok] > 1e-10).mean() < 1e-3
+
+
+def test_config5_full_size(G, O):
+    """BASELINE.json configs[4] at full size: 2048^2 grid, 2e8 particles (density ~ r^-2, thermal
+    momenta), one step of the coupled loop in bench.py's launch configuration: stable cell sort
+    (permutation bit-exact on all 2e8 keys), fused push + deposit + removal, 3 binomial filter passes +
+    normalisation.  A sample of 2e5 particles is pushed one by one by the oracle; J is compared on a
+    band of theta rows that the oracle deposits from exactly the particles that can reach it (a move
+    is shorter than one cell, the filter reaches 3 rows further): <= 1e-11 of the band's max."""
+    cfg = inputs.config(5)
+    p, dt, fields, ptc = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    ptc["w"][:] = 1e-6
+    n = len(ptc["x1"])
+    assert n == 200_000_000
+    ctx = G.Context(p, n)
+    f_t = [ctx.to_device(f) for f in fields]
+    A, B = G.Particles.from_numpy(ptc), G.Particles(n)
+    perm_t = torch.zeros(n, dtype=torch.int32, device="cuda")
+    ctx.sort(A, B, perm_t)
+    torch.cuda.synchronize()
+    perm = perm_t.cpu().numpy().view(np.uint32)
+    del perm_t
+    assert np.array_equal(perm, O.sort(ptc["cell"], ptc["flag"]))
+    n1 = torch.zeros(1, dtype=torch.int64, device="cuda")
+    F = ctx.zeros(3)
+    ctx.status.zero_()
+    ctx.push_deposit_compact(B, A, f_t, F, dt, n1)
+    ctx.finalize_current(F, 3)
+    torch.cuda.synchronize()
+    assert int(n1.item()) == n and int(ctx.status.item()) == 0
+    got = A.to_numpy()
+    rng = np.random.default_rng(5)
+    sample = np.sort(rng.choice(n, 200_000, replace=False))
+    src = perm[sample]
+    sub = {k: np.ascontiguousarray(v[src]) for k, v in ptc.items()}
+    ref = O.push(p, fields, sub, dt)
+    check_push(p, sub, ref, {k: got[k][sample] for k in got}, O, fields, dt, label="c5 full size")
+    # J on a band of rows: every particle whose old or new theta row lies within the band +- 6 rows
+    dth = math.pi / p["nth"]
+    j0, j1 = 1000, 1024
+    jo = np.floor(ptc["x2"] / dth).astype(np.int64)
+    jn = np.floor(got["x2"] / dth).astype(np.int64)           # sorted order
+    inv_sel = ((jn >= j0 - 8) & (jn <= j1 + 8))
+    sel_sorted = np.flatnonzero(inv_sel | ((jo[perm] >= j0 - 8) & (jo[perm] <= j1 + 8)))
+    srcb = perm[sel_sorted]
+    subb = {k: np.ascontiguousarray(v[srcb]) for k, v in ptc.items()}
+    refb = O.push(p, fields, subb, dt)
+    Jb = O.finalize_current(p, O.deposit(p, subb, refb, subb["w"], dt), 3)
+    Gd = p["ng"]
+    for c in range(3):
+        gotJ = ctx.to_host(F[c])[Gd + j0:Gd + j1 + 1, :]
+        refJ = Jb[c][Gd + j0:Gd + j1 + 1, :]
+        e = np.max(np.abs(gotJ - refJ)) / np.max(np.abs(refJ))
+        assert e <= 1e-11, (c, e)

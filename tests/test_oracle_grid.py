@@ -442,3 +442,173 @@ def test_spline3_gather_reproduces_linear_fields():
         got = np.array([oracle.gather(p, fields, x1[q], x2[q]) for q in range(n)])
     for k in range(6):
         assert np.allclose(got[:, k], exact[k], rtol=0, atol=1e-12), k
+
+
+# ------------------------------------------------------------------ first-order gather (G11/G12) and filter edges (S10)
+def _linear_fields(p, coef):
+    """six stored arrays with F(i, j) = a + b (i + s_r) + c (j + s_theta) at every stored index"""
+    G, nr, nth = p["ng"], p["nr"], p["nth"]
+    jj, ii = np.meshgrid(np.arange(-G, nth + G + 1), np.arange(-G, nr + G + 1), indexing="ij")
+    out = []
+    for (a, b, c), name in zip(coef, inputs.FIELD_NAMES):
+        sr, sth, _ = inputs.STAGGER[name]
+        out.append(np.ascontiguousarray(a + b * (ii + sr) + c * (jj + sth), dtype=np.float64))
+    return out
+
+
+def test_cic_gather_exact_on_linear_fields_per_lattice():
+    """PAPER.md:228, :297 'first order interpolation': bilinear weights on each component's OWN
+    staggered lattice reproduce a field that is linear in the index coordinates exactly.  A wrong
+    stagger offset, swapped x/y weights or a dropped corner shows up as an O(1) error."""
+    p = small_params(20, 16, 0.9)
+    rng = np.random.default_rng(5)
+    coef = rng.uniform(-2, 2, (6, 3))
+    fields = _linear_fields(p, coef)
+    dxi, dth = inputs.spacing(p)
+    for _ in range(200):
+        fx, fy = rng.uniform(0, p["nr"]), rng.uniform(1.0, p["nth"] - 1.0)   # away from the axis rows
+        got = oracle.gather(p, fields, p["xi_in"] + fx * dxi, fy * dth)
+        want = coef[:, 0] + coef[:, 1] * fx + coef[:, 2] * fy
+        assert np.allclose(got, want, rtol=0, atol=2e-13), (fx, fy, got - want)
+    # each component only sees its own array: perturbing one array changes one output
+    base = oracle.gather(p, fields, p["xi_in"] + 7.3 * dxi, 5.6 * dth)
+    for c in range(6):
+        f2 = [f.copy() for f in fields]
+        f2[c] += 1.0
+        d = oracle.gather(p, f2, p["xi_in"] + 7.3 * dxi, 5.6 * dth) - base
+        assert np.allclose(d, np.eye(6)[c], atol=1e-13)
+
+
+def test_cic_gather_axis_parity():
+    """G12: beyond the axis a component continues with its parity under theta -> -theta (r, phi
+    components even, theta components odd).  With random stored values the
+    interpolant must be mirror symmetric about theta = 0 and theta = pi, odd components must vanish
+    on the axis, and inside the first half cell a half-staggered even component must not depend on
+    theta."""
+    p = small_params(12, 10, 0.7)
+    rng = np.random.default_rng(6)
+    g = oracle.Grid(p)
+    fields = [rng.uniform(-1, 1, g.shape) for _ in range(6)]
+    G, nth = p["ng"], p["nth"]
+    for name in ("Dph", "Bth"):                     # axis nodes of D^phi, B^theta are zero (PAPER.md:132)
+        k = inputs.FIELD_NAMES.index(name)
+        fields[k][G, :] = 0.0
+        fields[k][G + nth, :] = 0.0
+    dxi, dth = inputs.spacing(p)
+    par = np.array([inputs.STAGGER[n][2] for n in inputs.FIELD_NAMES], dtype=float)
+    par[inputs.FIELD_NAMES.index("Dph")] = +1.0
+    for _ in range(100):
+        x1 = p["xi_in"] + rng.uniform(1, p["nr"] - 1) * dxi
+        t = rng.uniform(0.0, 1.9) * dth
+        up, dn = oracle.gather(p, fields, x1, t), oracle.gather(p, fields, x1, -t)
+        assert np.allclose(dn, par * up, atol=1e-14), (t / dth, dn, up)
+        up, dn = oracle.gather(p, fields, x1, math.pi - t), oracle.gather(p, fields, x1, math.pi + t)
+        assert np.allclose(dn, par * up, atol=1e-13), (t / dth, dn, up)
+    x1 = p["xi_in"] + 4.25 * dxi
+    on_axis = oracle.gather(p, fields, x1, 0.0)
+    for name in ("Dth", "Bth"):
+        assert abs(on_axis[inputs.FIELD_NAMES.index(name)]) < 1e-15
+    kBr = inputs.FIELD_NAMES.index("Br")            # half-staggered, even: flat across the axis
+    a = oracle.gather(p, fields, x1, 0.1 * dth)[kBr]
+    b = oracle.gather(p, fields, x1, 0.4 * dth)[kBr]
+    row0 = 0.75 * fields[kBr][g.ij(4, 0)] + 0.25 * fields[kBr][g.ij(5, 0)]
+    assert abs(a - b) < 1e-15 and abs(a - row0) < 1e-15
+
+
+def _filter_numpy(F, p, half_theta, parity):
+    """(1,2,1) x (1,2,1) / 16 on the physical rows: theta neighbours beyond the axis by parity,
+    radial neighbours beyond the first / last stored node clamped (S10), written with numpy slices."""
+    G, nr, nth = p["ng"], p["nr"], p["nth"]
+    jhi = nth - 1 if half_theta else nth
+    A = F[G:G + jhi + 1, :].copy()                   # rows 0..jhi, all stored columns
+    if half_theta:
+        lo, hi = parity * A[0], parity * A[jhi]      # row -1/2 mirrors row +1/2
+    else:
+        lo, hi = parity * A[1], parity * A[jhi - 1]  # row -1 mirrors row +1
+    T = np.vstack([lo, A, hi])
+    T = (T[:-2] + 2 * T[1:-1] + T[2:]) / 4.0
+    R = np.hstack([T[:, :1], T, T[:, -1:]])
+    R = (R[:, :-2] + 2 * R[:, 1:-1] + R[:, 2:]) / 4.0
+    out = F.copy()
+    out[G:G + jhi + 1, :] = R
+    return out
+
+
+def test_filter_pass_matches_numpy_convolution_including_edges():
+    """S10 on a random array, every physical row and every stored column (axis rows 0 and n_theta,
+    first and last radial guard), one and three passes, against a numpy convolution with parity
+    padding: pins the stencil weights, the parity sign per component and the radial clamp."""
+    p = small_params(14, 9, 0.6)
+    rng = np.random.default_rng(8)
+    g = oracle.Grid(p)
+    F0 = [rng.uniform(-1, 1, g.shape) for _ in range(3)]
+    A = oracle.areas(p)
+    area = [A["ADr"], A["ADth"], A["ADph"] * p["dphi"]]
+    folded = oracle.fold_current(p, [x.copy() for x in F0])
+    for passes in (1, 3):
+        J = oracle.finalize_current(p, [x.copy() for x in F0], passes)
+        ref = [x.copy() for x in folded]
+        for _ in range(passes):
+            ref = [_filter_numpy(ref[0], p, False, +1.0), _filter_numpy(ref[1], p, True, -1.0),
+                   _filter_numpy(ref[2], p, False, +1.0)]
+        for c in range(3):
+            ok = area[c] > 0
+            assert np.allclose((J[c] * area[c])[ok], ref[c][ok], rtol=1e-13, atol=1e-14), (passes, c)
+
+
+def test_field_step_threads_bit_identical():
+    """The OpenMP loops of the oracle's field step run over grid rows with no reduction: one thread
+    and all threads must give the same bits (areas, circulations, a full N = 7 step with damping)."""
+    p = small_params(40, 28, 0.9, damp_cells=6, damp_coef=1.0)
+    rng = np.random.default_rng(12)
+    f0 = inputs.fill_guards(p, inputs.perturb(inputs.analytic_fields(p, "wald"), 1e-2, rng))
+    J = [rng.uniform(-1e-3, 1e-3, f0[0].shape) for _ in range(3)]
+    dt = inputs.courant_dt(p)
+    old = oracle.set_num_threads(1)
+    try:
+        A1 = oracle.areas(p)
+        C1 = oracle.circulation(p, f0)
+        F1 = oracle.field_step(p, [f.copy() for f in f0], J, dt, bg=f0)
+        oracle.set_num_threads(max(2, old))
+        A2 = oracle.areas(p)
+        C2 = oracle.circulation(p, f0)
+        F2 = oracle.field_step(p, [f.copy() for f in f0], J, dt, bg=f0)
+    finally:
+        oracle.set_num_threads(old)
+    for k in A1:
+        assert np.array_equal(A1[k], A2[k]), k
+    for a, b in zip(C1 + F1, C2 + F2):
+        assert np.array_equal(a, b)
+
+
+def test_damping_layer_properties():
+    """PAPER.md:138 gives no profile (reading G14); whatever the profile, an absorbing layer must
+    (1) leave every column inside i <= nr - damp_cells bit-exactly alone, (2) pull the fields towards
+    the background, never past it and never away from it (0 <= lambda <= 1), (3) act monotonically
+    more strongly outwards, (4) be the identity on a field that equals the background, and (5) vanish
+    continuously at its inner edge.  dt = 0 isolates the damping stage of the step."""
+    p = small_params(40, 10, 0.9, damp_cells=12, damp_coef=0.7, field_iters=2)
+    g = oracle.Grid(p)
+    rng = np.random.default_rng(3)
+    bg = inputs.fill_guards(p, [rng.uniform(-1, 1, g.shape) for _ in range(6)])
+    f = inputs.fill_guards(p, [b + rng.uniform(0.5, 1.5, g.shape) for b in bg])    # f - bg > 0 everywhere
+    out = oracle.field_step(p, [x.copy() for x in f], None, 0.0, bg=bg)
+    G, nr, nth = p["ng"], p["nr"], p["nth"]
+    i0 = nr - p["damp_cells"]
+    for c, name in enumerate(inputs.FIELD_NAMES):
+        sr, sth, _ = inputs.STAGGER[name]
+        jlo, jhi = (1, nth - 1) if name in ("Dph", "Bth") else (0, nth if sth == 0.0 else nth - 1)
+        ihi = nr if sr == 0.0 else nr - 1
+        rows = slice(G + jlo, G + jhi + 1)
+        assert np.array_equal(out[c][rows, G:G + i0 + 1], f[c][rows, G:G + i0 + 1]), name          # (1)
+        lam = (out[c][rows, G + i0 + 1:G + ihi + 1] - bg[c][rows, G + i0 + 1:G + ihi + 1]) / \
+              (f[c][rows, G + i0 + 1:G + ihi + 1] - bg[c][rows, G + i0 + 1:G + ihi + 1])
+        assert np.all(lam >= 0.0) and np.all(lam <= 1.0), name                                     # (2)
+        assert np.all(np.diff(lam, axis=1) <= 1e-15), name                                         # (3)
+        assert np.all(lam[:, 0] > 0.999) and np.all(lam[:, -1] < 0.5), name                        # (5), strong at the edge
+        assert np.allclose(lam, lam[:1, :], atol=1e-14), name                                      # same for every row
+    same = oracle.field_step(p, [x.copy() for x in bg], None, 0.0, bg=bg)                          # (4)
+    for c, name in enumerate(inputs.FIELD_NAMES):
+        sth = inputs.STAGGER[name][1]
+        jlo, jhi = (1, nth - 1) if name in ("Dph", "Bth") else (0, nth if sth == 0.0 else nth - 1)
+        assert np.array_equal(same[c][G + jlo:G + jhi + 1, G:G + nr], bg[c][G + jlo:G + jhi + 1, G:G + nr]), name

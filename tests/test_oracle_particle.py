@@ -434,6 +434,13 @@ def test_pair_production_conserves_fido_momentum_and_energy():
     assert ov2 and len(out2["x1"]) == n + 5
     for k in out2:
         assert np.array_equal(out2[k][n:], out[k][n:n + 5]), k
+    # P5: the events whose child found no room did not happen -- those parents are untouched (same
+    # momentum, same species), so no charge or momentum disappears; the first five events are the
+    # ones of the unbounded run
+    kept, dropped = par[:5], par[5:]
+    for k in ("u1", "u2", "u3", "flag"):
+        assert np.array_equal(out2[k][:n][dropped], ptc[k][dropped]), k
+        assert np.array_equal(out2[k][:n][kept], out[k][:n][kept]), k
 
 
 # ------------------------------------------------------------------ Vay pusher in the FIDO frame
@@ -515,3 +522,62 @@ def test_push_with_vay_option_uses_vay():
     ub = oracle.vay(p["a"], p["M"], r, th, [ptc["u1"][k], ptc["u2"][k], ptc["u3"][k]], D6[:3], D6[3:], sgn, dt)
     yn = oracle.geodesic(p["a"], p["M"], 3, np.array([r, th, ptc["x3"][k], *ub]), dt)
     assert abs(math.log(yn[0]) - nv["x1"][k]) < 1e-15 and abs(yn[3] - nv["u1"][k]) < 1e-15
+
+
+# ------------------------------------------------------------------ S4.5-S4.7: reflection, removal flag, new cell
+def test_push_reflection_removal_and_cell_on_hand_built_particles():
+    """PAPER.md:136 ('correct reflection'), :138 (removal at the radial boundaries).  With D = B = 0
+    the Boris step is the identity, so orc_push = geodesic step (pinned above) + the post-processing
+    under test.  Hand-built particles: one crosses theta = 0, one crosses theta = pi, one ends below
+    xi_in, one at / beyond xi_out, one stays inside.  Expected: theta -> -theta (2 pi - theta) with
+    u_theta flipped and x2dep the un-reflected angle; flag bit 1 and cell 0xFFFFFFFF exactly for the
+    two leavers; cell = floor(theta / dtheta) * nr + floor((xi - xi_in) / dxi) for the others."""
+    import inputs
+    p = inputs.grid_params(32, 24, 0.9, r_out=20.0)
+    a, M = p["a"], 1.0
+    g = oracle.Grid(p)
+    dxi, dth = inputs.spacing(p)
+    fields = [np.zeros(g.shape) for _ in range(6)]
+    dt = 0.02
+    r_in, r_out = math.exp(p["xi_in"]), math.exp(p["xi_out"])
+    rows = [  # r, theta, phi, u_r, u_theta, u_phi
+        (5.0, 2e-3, 0.3, 0.0, -8.0, 0.0),             # crosses theta = 0 (u_theta < 0; no u_phi: no centrifugal wall)
+        (6.0, math.pi - 2e-3, 1.0, 0.2, 9.0, 0.0),    # crosses theta = pi
+        (r_in * 1.004, 1.1, 0.0, -30.0, 0.1, 0.2),    # falls below r_in
+        (r_out * 0.9995, 2.0, 0.0, 40.0, 0.0, 0.1),   # leaves through r_out
+        (7.0, 1.3, 2.0, 0.5, -0.7, 1.5),              # stays inside
+    ]
+    y = np.array(rows)
+    y[:, 0] = np.exp(np.log(y[:, 0]))               # the state stores xi = ln r: start from r = exp(xi)
+    ptc = {"x1": np.log(y[:, 0]), "x2": y[:, 1].copy(), "x3": y[:, 2].copy(), "u1": y[:, 3].copy(),
+           "u2": y[:, 4].copy(), "u3": y[:, 5].copy(), "flag": np.array([0, 1, 0, 1, 0], dtype=np.uint32)}
+    out = oracle.push(p, fields, ptc, dt)
+    geo = np.array([oracle.geodesic(a, M, 3, yy, dt) for yy in y])
+    th_new = geo[:, 1]
+    assert th_new[0] < 0 and th_new[1] > math.pi                   # the cases are what they claim to be
+    assert math.log(geo[2, 0]) < p["xi_in"] and math.log(geo[3, 0]) >= p["xi_out"]
+    # un-reflected angle for the deposit, mirrored angle and flipped u_theta in the state
+    assert np.array_equal(out["x2dep"], th_new)
+    assert out["x2"][0] == -th_new[0] and out["u2"][0] == -geo[0, 4]
+    assert out["x2"][1] == 2 * math.pi - th_new[1] and out["u2"][1] == -geo[1, 4]
+    for k in (2, 3, 4):
+        assert out["x2"][k] == th_new[k] and out["u2"][k] == geo[k, 4]
+    assert np.all((out["x2"] >= 0) & (out["x2"] <= math.pi))
+    assert np.array_equal(out["x1"], np.log(geo[:, 0])) and np.array_equal(out["x3"], geo[:, 2])
+    assert np.array_equal(out["u1"], geo[:, 3]) and np.array_equal(out["u3"], geo[:, 5])
+    # removal flag (bit 1) and cell
+    assert list(out["flag"]) == [0, 1, 0 | 2, 1 | 2, 0]
+    assert out["cell"][2] == 0xFFFFFFFF and out["cell"][3] == 0xFFFFFFFF
+    for k in (0, 1, 4):
+        ic = int(math.floor((out["x1"][k] - p["xi_in"]) / dxi))
+        jc = int(math.floor(out["x2"][k] / dth))
+        assert 0 <= ic < p["nr"] and 0 <= jc < p["nth"]
+        assert out["cell"][k] == jc * p["nr"] + ic
+    assert out["cell"][0] // p["nr"] == 0 and out["cell"][1] // p["nr"] == p["nth"] - 1   # rows next to the axes
+    # a particle already flagged removed is passed through untouched
+    ptc2 = {k: v.copy() for k, v in ptc.items()}
+    ptc2["flag"][4] |= 2
+    out2 = oracle.push(p, fields, ptc2, dt)
+    for k in ("x1", "x2", "x3", "u1", "u2", "u3"):
+        assert out2[k][4] == ptc[k][4]
+    assert out2["flag"][4] == 2 and out2["cell"][4] == 0xFFFFFFFF
