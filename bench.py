@@ -154,6 +154,8 @@ def parse(argv=None):
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    ap.add_argument("--host-logic-check", action="store_true",
+                    help="CPU/gloo run of the multi-rank host logic only (used by the tests)")
     return ap.parse_args(argv)
 
 
@@ -223,7 +225,7 @@ def workload(args, rank):
                   2: ("r2", ("mj_tail", 1.0, 0.1, 10.0, 1e4), True, 20_000_000, 1),
                   3: ("crowded", ("loguniform", 0.1, 1e5), False, 100_000_000, 2),
                   5: ("r2", ("mj", 0.1), False, 200_000_000, 4)}[k]
-        cfg["particles"] = inputs.make_particles(cfg["params"], n or recipe[3], recipe[4] + 7919 * rank,
+        cfg["particles"] = inputs.make_particles(cfg["params"], n or recipe[3], rank_seed(k, rank),
                                                  recipe[0], recipe[1], pairs=recipe[2])
     else:
         cfg = inputs.config(k, nr=g, nth=g, n=n)
@@ -233,6 +235,50 @@ def workload(args, rank):
 # plasma weight used by the timed loop: the field step consumes J, so the macro-particle
 # weight is scaled down to keep |J dt| << |B|; parity tests use w = 1.
 BENCH_WEIGHT = 1e-9
+
+
+def reduce_over_ranks(ms, units, world, dist, device):
+    """timing rule of the contract: MAX of the device time over ranks, SUM of the units processed"""
+    if world <= 1:
+        return float(ms), float(units)
+    import torch
+    t = torch.tensor([float(ms)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    u = torch.tensor([float(units)], dtype=torch.float64, device=device)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(t.item()), float(u.item())
+
+
+def rank_seed(config, rank):
+    """every rank draws its own particle set (weak scaling): the recipe's seed + 7919 rank"""
+    return {1: 0, 2: 1, 3: 2, 5: 4}[config] + 7919 * rank
+
+
+def run_host_logic_check(args):
+    """`--host-logic-check`: the multi-rank HOST logic of this script (self-launch of N ranks,
+    rendezvous, per-rank seeds, the single all-reduce of the contiguous flux block, max-time / sum-units
+    aggregation, rank 0 printing the line) on CPU with the gloo backend -- what tests/ can run without
+    GPUs.  No kernel runs and no throughput is measured."""
+    import torch
+    import torch.distributed as dist
+    from paper_2503_04558_b200 import sharding
+    rank, world = env_int("RANK", 0), env_int("WORLD_SIZE", 1)
+    if world > 1:
+        dist.init_process_group("gloo")
+    block = torch.full((3, 5, 16), float(rank + 1), dtype=torch.float64)
+    sharding.allreduce_flux(block)
+    ms, units = reduce_over_ranks(10.0 + rank, 1000.0 * (rank + 1), world, dist, "cpu")
+    lo, hi = sharding.shard_range(1001, rank, world)
+    sizes = torch.zeros(world, dtype=torch.float64)
+    sizes[rank] = hi - lo
+    if world > 1:
+        dist.all_reduce(sizes)
+    if rank == 0:
+        print(json.dumps({"host_logic_check": True, "n_gpus": world, "ms_max": ms, "units_sum": units,
+                          "flux_sum": float(block[0, 0, 0]), "seeds": [rank_seed(args.config, r) for r in range(world)],
+                          "shards": [int(x) for x in sizes]}))
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def run_ours(args):
@@ -343,10 +389,6 @@ def run_ours(args):
     tw1 = time.time()
     launches = ctx.kernel_launches() - launches0
     ms_total = e0.elapsed_time(e1)
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
     clocks = ClockSampler.summarise(sampler.window(tw0, tw1)) if sampler else None
 
     # particles actually pushed per timed step (alive at the start of the step)
@@ -359,11 +401,7 @@ def run_ours(args):
         pushed = [int(al[s]) if fused else (n if s == 0 else int(al[s - 1])) for s in range(W, W + K)]
     else:
         pushed = [n] * K
-    units = float(sum(pushed))
-    if world > 1:
-        t = torch.tensor([units], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.SUM)
-        units = float(t.item())
+    ms_total, units = reduce_over_ranks(ms_total, float(sum(pushed)), world, dist, "cuda")
     value = units / (ms_total * 1e-3)
 
     phases = {}
@@ -591,6 +629,8 @@ def run_e2e(args, ctx, grpic, state, fields0, flux, dt, filt, bg, world, dist):
     host["n"] = n
     hJ = [torch.empty(f.shape, dtype=f.dtype).pin_memory() for f in flux]
     fields = [f.clone() for f in fields0]
+    if world > 1:     # the ranks' fluxes are summed inside the step (one all-reduce on the stream)
+        ctx.set_flux_exchange(lambda block: dist.all_reduce(block, op=dist.ReduceOp.SUM))
     ctx.step_host(host, fields, dt, host_J=hJ, background=bg, filter_passes=filt, chunk=args.e2e_chunk)   # warm-up, allocates staging
     torch.cuda.synchronize()
     units, h2d, d2h = 0, 0, 0
@@ -610,12 +650,9 @@ def run_e2e(args, ctx, grpic, state, fields0, flux, dt, filt, bg, world, dist):
     ms = max(e0.elapsed_time(e1), wall_ms)            # the call blocks: wall clock covers the copies home
     note = ""
     if world > 1:     # ranks step their own particle shard; max time over ranks, units summed
-        t = torch.tensor([ms, -float(units)], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t[:1], op=dist.ReduceOp.MAX)
-        u = torch.tensor([float(units)], dtype=torch.float64, device="cuda")
-        dist.all_reduce(u, op=dist.ReduceOp.SUM)
-        ms, units = float(t[0].item()), float(u.item())
-        note = " (N > 1: each rank steps its own shard with its own flux; no cross-rank flux sum in this leg)"
+        ctx.set_flux_exchange(None)
+        ms, units = reduce_over_ranks(ms, units, world, dist, "cuda")
+        note = " (N > 1: each rank steps its own shard; the fluxes are summed over ranks inside the step)"
     return {"value": float(units) / (ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d // KE),
             "d2h_bytes_per_step": int(d2h // KE), "steps": KE, "ms_per_step": ms / KE,
             "path": "grpic_step_host: pinned host SoA -> chunked H2D | push+deposit+compaction | D2H of the "
@@ -718,6 +755,8 @@ def main(argv=None):
     if a.gpus > 1 and "WORLD_SIZE" not in os.environ and a.config != 4:
         # `python bench.py --gpus N` without a launcher: start the N ranks ourselves
         return subprocess.call(relaunch_argv(argv, a.gpus))
+    if a.host_logic_check:
+        return run_host_logic_check(a)
     if a.config == 4:
         return run_field_only(a)
     return run_ours(a)

@@ -155,6 +155,15 @@ int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_
                                const grpic_fields* fields, grpic_current* flux, double dt,
                                int64_t* n_alive, uint32_t* status, void* stream);
 
+/* Multi-GPU hook of grpic_step_host (partitioning A: particles sharded over ranks, grid
+ * replicated): when set, the callback is invoked once per grpic_step_host call, after the last
+ * particle chunk has been deposited and before the current is finalised, with the DEVICE pointer of
+ * the context's three flux arrays (contiguous, 3 x rows x pitch doubles) and the caller's stream.  It
+ * must sum them over the ranks in stream order (e.g. one ncclAllReduce on that stream) and return 0;
+ * any other value aborts the step with GRPIC_ERR_CUDA.  fn = NULL removes the hook. */
+typedef int (*grpic_flux_exchange_fn)(void* user, double* flux3, size_t n_doubles, void* stream);
+int grpic_set_flux_exchange(grpic_ctx* ctx, grpic_flux_exchange_fn fn, void* user);
+
 /* END-TO-END step with the particle state in HOST memory (the one call that takes host
  * pointers): host_ptc (HOST SoA; pinned memory makes the copies asynchronous), host_J (HOST,
  * grid layout, nullable) and host_status (HOST word, nullable); `fields` / `background` stay

@@ -150,6 +150,8 @@ int grpic_create(const grpic_params* p, grpic_ctx** out) {
   ctx->ws_bytes = 0;
   ctx->host_step = nullptr;
   ctx->removed_counter = nullptr;
+  ctx->flux_exchange = nullptr;
+  ctx->flux_exchange_user = nullptr;
   cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
   GridDev& g = ctx->g;
   g.a = p->a; g.M = p->M; g.a2 = p->a * p->a; g.twoM = 2.0 * p->M;
@@ -240,6 +242,13 @@ size_t grpic_workspace_bytes(const grpic_ctx* ctx, int64_t n_particles) {
 int grpic_set_removed_counter(grpic_ctx* ctx, unsigned long long* device_counter) {
   if (!ctx) return GRPIC_ERR_ARG;
   ctx->removed_counter = device_counter;
+  return GRPIC_OK;
+}
+
+int grpic_set_flux_exchange(grpic_ctx* ctx, grpic_flux_exchange_fn fn, void* user) {
+  if (!ctx) return GRPIC_ERR_ARG;
+  ctx->flux_exchange = fn;
+  ctx->flux_exchange_user = user;
   return GRPIC_OK;
 }
 

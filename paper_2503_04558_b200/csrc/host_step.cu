@@ -169,6 +169,9 @@ extern "C" int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_
   }
   if (nchunks >= 1) { rc = finish(nchunks - 1); if (rc != GRPIC_OK) return fail(rc); }
 
+  // multi-GPU: sum the fluxes of the ranks' particle shards (one collective on the caller's stream)
+  if (ctx->flux_exchange && ctx->flux_exchange(ctx->flux_exchange_user, S->flux[0], 3 * n2, stream) != 0)
+    return fail(GRPIC_ERR_CUDA);
   // grid part of the step on the caller's stream, overlapping the last copies home
   rc = grpic_finalize_current(ctx, &flux, filter_passes, st);
   if (rc != GRPIC_OK) return fail(rc);

@@ -46,7 +46,7 @@ class CurrentC(C.Structure):
 
 
 EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_areas",
-           "grpic_workspace_bytes", "grpic_set_workspace", "grpic_set_removed_counter", "grpic_push_deposit",
+           "grpic_workspace_bytes", "grpic_set_workspace", "grpic_set_removed_counter", "grpic_set_flux_exchange", "grpic_push_deposit",
            "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
@@ -172,6 +172,31 @@ class Context:
         self._removed = counter          # keep the tensor alive while the library holds its pointer
         ptr = C.c_void_p(counter.data_ptr()) if counter is not None else None
         _check(load().grpic_set_removed_counter(self.h, ptr))
+
+    def set_flux_exchange(self, fn):
+        """fn(flux_block) or None.  flux_block: torch view [3, rows, pitch] of the context's own flux
+        arrays inside grpic_step_host; fn must sum it over the ranks in stream order (e.g.
+        torch.distributed.all_reduce on the current stream)."""
+        if fn is None:
+            self._fx_cb = None
+            _check(load().grpic_set_flux_exchange(self.h, None, None))
+            return
+        rows, pitch = self.rows, self.pitch
+
+        class _Dev:                                   # raw device pointer -> torch tensor, no copy
+            def __init__(self, ptr, n):
+                self.__cuda_array_interface__ = {"shape": (n,), "typestr": "<f8", "data": (ptr, False), "version": 2}
+
+        def cb(user, ptr, n, stream):
+            try:
+                t = torch.as_tensor(_Dev(ptr, int(n)), device="cuda").view(3, rows, pitch)
+                fn(t)
+                return 0
+            except Exception:                          # never let an exception cross the C boundary
+                return 1
+        proto = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_size_t, C.c_void_p)
+        self._fx_cb = proto(cb)                        # keep the thunk alive
+        _check(load().grpic_set_flux_exchange(self.h, self._fx_cb, None))
 
     def close(self):
         if self.h:

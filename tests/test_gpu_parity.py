@@ -1137,3 +1137,56 @@ def test_config5_full_size(G, O):
         refJ = Jb[c][Gd + j0:Gd + j1 + 1, :]
         e = np.max(np.abs(gotJ - refJ)) / np.max(np.abs(refJ))
         assert e <= 1e-11, (c, e)
+
+
+def test_step_host_flux_exchange_hook(G, O):
+    """grpic_set_flux_exchange: the multi-GPU hook of grpic_step_host is called exactly once per step,
+    between the deposit and the finalisation, with the context's contiguous 3-array flux block.  One GPU
+    stands in for N identical ranks: a hook that triples the block (the sum over three equal ranks) must
+    give exactly the oracle's J for three copies of the particle set, and the fields that follow."""
+    p = inputs.grid_params(40, 32, 0.9, field_iters=2)
+    dt = inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "wald")
+    n = 5000
+    ptc = inputs.make_particles(p, n, 5, "r2", ("loguniform", 0.1, 10.0))
+    ptc["w"][:] = 1e-3
+    ctx = G.Context(p, n)
+    f_t = [ctx.to_device(f) for f in fields]
+    host = {k: torch.from_numpy(v.copy() if v.dtype != np.uint32 else v.view(np.int32).copy()).pin_memory()
+            for k, v in ptc.items()}
+    host["n"] = n
+    hJ = [torch.zeros((ctx.rows, ctx.pitch), dtype=torch.float64).pin_memory() for _ in range(3)]
+    calls = []
+
+    def hook(block):
+        calls.append(tuple(block.shape))
+        block.mul_(3.0)
+    ctx.set_flux_exchange(hook)
+    ctx.step_host(host, f_t, dt, host_J=hJ)
+    ctx.set_flux_exchange(None)
+    assert calls == [(3, ctx.rows, ctx.pitch)]
+    ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
+    Jref = O.finalize_current(p, [3.0 * F for F in Fref], 0)
+    fref = O.field_step(p, [f.copy() for f in fields], Jref, dt)
+    for c in range(3):
+        assert grid_err(Jref[c], ctx.to_host(hJ[c].cuda())) <= 1e-11, c
+    for c in range(6):
+        assert grid_err(fref[c], ctx.to_host(f_t[c])) <= 1e-11, c
+    ctx.step_host(host, f_t, dt, host_J=hJ)            # hook removed: not called again
+    assert len(calls) == 1
+
+
+def test_bench_two_ranks_if_two_gpus():
+    """bench.py --gpus 2 on a box with at least two devices: two NCCL ranks, n_gpus = 2 on the line."""
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs (the pool's boxes expose one)")
+    import json
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "2", "--steps", "3", "--warmup", "3",
+                          "--particles", "2000000", "--grid", "512", "--no-cpu-baseline", "--e2e-steps", "1"],
+                         capture_output=True, text=True, timeout=900, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads([l for l in out.stdout.splitlines() if l.startswith("{")][-1])
+    assert d["n_gpus"] == 2 and d["value"] > 0 and "allreduce" in d["phases_ms"]

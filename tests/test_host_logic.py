@@ -127,3 +127,49 @@ def test_bench_reference_arm_prints_contract_line():
     env = dict(os.environ, RANK="1", WORLD_SIZE="2")
     out1 = subprocess.run(cmd, capture_output=True, text=True, timeout=300, check=True, env=env).stdout.strip()
     assert out1 == ""
+
+
+def test_bench_gpus_flag_starts_n_ranks_gloo():
+    """`python bench.py --gpus 2` with no launcher in the environment starts the two ranks itself
+    (torch.distributed.run on 127.0.0.1) and runs bench.py's OWN multi-rank host logic: rendezvous,
+    per-rank seeds, ONE all-reduce of the contiguous 3-array flux block, max-time / sum-units
+    aggregation, rank 0 alone printing the line (CPU stand-in with gloo)."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--host-logic-check"],
+                         capture_output=True, text=True, timeout=300, env=env, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1                                  # rank 1 prints nothing
+    d = json.loads(lines[0])
+    assert d["n_gpus"] == 2 and d["ms_max"] == 11.0 and d["units_sum"] == 3000.0
+    assert d["flux_sum"] == 3.0                             # (rank 0: 1) + (rank 1: 2), one collective
+    assert d["seeds"] == [2, 2 + 7919] and d["shards"] == [501, 500]
+
+
+def test_bench_relaunch_command_line():
+    sys.path.insert(0, ROOT)
+    import bench
+    cmd = bench.relaunch_argv(["--gpus", "4", "--steps", "5"], 4, port=12345)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"]
+    assert cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "12345"
+    assert cmd[-4:] == ["--gpus", "4", "--steps", "5"] and cmd[-5].endswith("bench.py")
+
+
+def test_allreduce_flux_uses_one_collective_for_a_block(monkeypatch):
+    """sharding.allreduce_flux on the contiguous [3, rows, pitch] block (or on its three views) issues
+    exactly one all-reduce; three separate arrays fall back to three."""
+    import torch
+    import torch.distributed as dist
+    calls = []
+    monkeypatch.setattr(dist, "is_initialized", lambda: True)
+    monkeypatch.setattr(dist, "get_world_size", lambda: 2)
+    monkeypatch.setattr(dist, "all_reduce", lambda t, op=None: calls.append(t.numel()))
+    block = torch.zeros(3, 4, 8, dtype=torch.float64)
+    sharding.allreduce_flux(block)
+    sharding.allreduce_flux(list(block.unbind(0)))
+    assert calls == [96, 96]
+    calls.clear()
+    sharding.allreduce_flux([torch.zeros(4, 8) for _ in range(3)])
+    assert calls == [32, 32, 32]
