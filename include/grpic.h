@@ -248,6 +248,15 @@ int grpic_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* ou
  * divide = 0 returns rho*dV.  Overwrites `rho`. */
 int grpic_deposit_rho(grpic_ctx* ctx, const grpic_particles* ptc, double* rho, int32_t divide, void* stream);
 
+/* Diagnostics in Boyer-Lindquist coordinates and in the FIDO frame ((A6)-(A7)): for
+ * every particle k < ptc->n writes  E_inf[k] = -u_t = alpha^2 u^0 - beta^r u_r  (energy at infinity),
+ * gamma_fido[k] = alpha u^0,  ur_bl[k] = u_r^KS - (2 M r E_inf - a u_phi)/Delta  (covariant radial
+ * momentum in BL; u_t, u_theta, u_phi are the same in both systems) and  phi_bl[k] = phi_KS -
+ * a/(2 sqrt(M^2-a^2)) ln|(r-r_+)/(r-r_-)|.  Output arrays are caller-owned DEVICE arrays of length
+ * >= ptc->n, each may be NULL; removed particles get NaN.  The particle arrays are not modified. */
+int grpic_ks_to_bl(grpic_ctx* ctx, const grpic_particles* ptc, double* E_inf, double* gamma_fido,
+                   double* ur_bl, double* phi_bl, void* stream);
+
 /* Roofline denominator: measured FP64 pipe throughput of this device.  Runs a register-only
  * kernel of independent DFMA chains on every SM (blocking, ~10 ms) and writes the achieved
  * FP64 instructions (lane-operations) per second to the HOST double *dfma_per_second. */

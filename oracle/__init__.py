@@ -315,6 +315,15 @@ def shape(x):
     return float(lib().orc_shape(C.c_double(x)))
 
 
+def ks_to_bl(a, M, x1, th, ph, u, eps=1.0):
+    """(E_inf, Gamma_FIDO, u_r^BL, phi_BL) of one Kerr-Schild particle state"""
+    u = np.ascontiguousarray(u, dtype=np.float64)
+    out = np.zeros(4)
+    lib().orc_ks_to_bl(C.c_double(a), C.c_double(M), C.c_double(x1), C.c_double(th), C.c_double(ph), _d(u),
+                       C.c_double(eps), _d(out))
+    return out
+
+
 def set_num_threads(n):
     """OpenMP threads of the oracle's parallel loops; returns the previous setting."""
     lib().orc_set_num_threads.restype = C.c_int

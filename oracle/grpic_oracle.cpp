@@ -21,6 +21,8 @@
 //   orc_circulation/field div B exactly preserved; div D - rho preserved; Wald/monopole
 //                         stationarity ~ Delta^2; Heun limit / order in dt
 //   orc_sort/orc_compact  = std::stable_sort / order-preserving filter (library definition)
+//   orc_ks_to_bl          Boyer-Lindquist normalisation g_BL^{mu nu} u_mu u_nu = -eps with the textbook BL
+//                         inverse metric; (A7) differentiated against (A6); u_i = 0 gives Gamma = 1
 //   orc_sort_interleaved  numpy lexsort of the defining tuple; hand-built example; B = 1 reduces to orc_sort
 //   shape option 3        cubic B-spline: partition of unity, moments, C2 knots; continuity to
 //                         round-off with the spline in rho and fluxes; exact gather of linear fields
@@ -1068,6 +1070,26 @@ int64_t orc_pair_production(const orc_params* p, int64_t n, int64_t capacity, do
     flag[k] = parent_flag;
   }
   return m;
+}
+
+// Boyer-Lindquist / FIDO diagnostics of a Kerr-Schild particle state ((A6), (A7)).
+// out[4] = { E_inf = -u_t, Gamma_FIDO = alpha u^0, u_r^BL, phi_BL }.
+//   -u_t = alpha^2 u^0 - beta^r u_r                      (u_t = g_{t mu} u^mu in the 3+1 split)
+//   (A6) dt_KS = dt_BL + 2Mr/Delta dr, dphi_KS = dphi_BL + a/Delta dr  =>  covariant components transform
+//   with the transposed Jacobian: u_r^BL = u_r^KS + (2Mr/Delta) u_t + (a/Delta) u_phi, others unchanged.
+//   (A7) phi_KS = phi_BL + a/(2 sqrt(M^2-a^2)) ln|(r - r_+)/(r - r_-)|.
+void orc_ks_to_bl(double a, double M, double x1, double th, double ph, const double u[3], double eps,
+                  double* out) {
+  const double r = std::exp(x1);
+  const Metric m = metric(a, M, r, th);
+  const double u0 = std::sqrt(eps + norm_up(m, u)) / m.alpha;
+  const double E = m.alpha * m.alpha * u0 - m.beta_r * u[0];
+  const double Delta = r * r - 2.0 * M * r + a * a;
+  const double root = std::sqrt(M * M - a * a);
+  out[0] = E;
+  out[1] = m.alpha * u0;
+  out[2] = u[0] + (2.0 * M * r / Delta) * (-E) + (a / Delta) * u[2];
+  out[3] = ph - (root > 0.0 ? a / (2.0 * root) * std::log(std::fabs((r - (M + root)) / (r - (M - root)))) : 0.0);
 }
 
 double orc_shape(double x) { return shape(x); }

@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libgrpic.so")
-SOURCES = ["api.cu", "push_deposit.cu", "field.cu", "current.cu", "sort.cu", "host_step.cu", "pair.cu", "push_spline3.cu"]
+SOURCES = ["api.cu", "push_deposit.cu", "field.cu", "current.cu", "sort.cu", "host_step.cu", "pair.cu", "push_spline3.cu", "diagnostics.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--use_fast_math=false"]
 
@@ -26,7 +26,7 @@ def _nvcc():
 
 def build(force=False, verbose=False):
     srcs = [os.path.join(CSRC, s) for s in SOURCES]
-    deps = srcs + [os.path.join(CSRC, "grpic_internal.cuh"), os.path.join(CSRC, "push_math.cuh"),
+    deps = srcs + [os.path.join(CSRC, "grpic_internal.cuh"), os.path.join(CSRC, "push_math.cuh"), os.path.join(CSRC, "poly_tables.cuh"),
                    os.path.join(HERE, "..", "include", "grpic.h")]
     if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB

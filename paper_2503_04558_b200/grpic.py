@@ -49,7 +49,7 @@ EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_area
            "grpic_workspace_bytes", "grpic_set_workspace", "grpic_set_removed_counter", "grpic_set_flux_exchange", "grpic_push_deposit",
            "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
-           "grpic_circulation", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
+           "grpic_circulation", "grpic_ks_to_bl", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
 
 _lib = None
@@ -350,6 +350,13 @@ class Context:
         _check(load().grpic_compact(self.h, C.byref(a), C.byref(b),
                                     C.cast(C.c_void_p(n_alive.data_ptr()), C.POINTER(C.c_int64)), _stream()))
         dst.n = src.n
+
+    def ks_to_bl(self, ptc):
+        """(E_inf, gamma_fido, ur_bl, phi_bl): four float64 device tensors of length ptc.n"""
+        out = [torch.empty(max(ptc.n, 1), dtype=torch.float64, device="cuda") for _ in range(4)]
+        ps = ptc.struct()
+        _check(load().grpic_ks_to_bl(self.h, C.byref(ps), *[_ptr(t) for t in out], _stream()))
+        return [t[:ptc.n] for t in out]
 
     def measure_fp64_peak(self):
         """measured FP64 pipe rate of this device, FP64 instructions (lane-ops) per second"""

@@ -581,3 +581,42 @@ def test_push_reflection_removal_and_cell_on_hand_built_particles():
     for k in ("x1", "x2", "x3", "u1", "u2", "u3"):
         assert out2[k][4] == ptc[k][4]
     assert out2["flag"][4] == 2 and out2["cell"][4] == 0xFFFFFFFF
+
+
+# ------------------------------------------------------------------ Boyer-Lindquist / FIDO diagnostics ((A6), (A7))
+def test_ks_to_bl_diagnostics():
+    """orc_ks_to_bl: (1) the transformed four-momentum (u_t, u_r^BL, u_theta, u_phi) is normalised with
+    the TEXTBOOK Boyer-Lindquist inverse metric, g^{mu nu} u_mu u_nu = -eps, for massive particles and
+    photons, inside and outside the ergosphere; (2) (A7) differentiates to (A6): d(phi_KS - phi_BL)/dr =
+    a / Delta; (3) a particle at rest in the FIDO frame has Gamma = 1; (4) E_inf is the quantity the
+    geodesic integrator conserves (same number along an orbit to the integrator's accuracy)."""
+    rng = np.random.default_rng(9)
+    for a in (0.0, 0.5, 0.998):
+        rh = 1.0 + math.sqrt(1.0 - a * a)
+        for _ in range(40):
+            r, th = rng.uniform(1.05 * rh, 20.0), rng.uniform(0.2, math.pi - 0.2)
+            u = rng.normal(size=3) * rng.choice([0.1, 3.0, 50.0])
+            for eps in (1.0, 0.0):
+                E, Gam, urb, phb = oracle.ks_to_bl(a, 1.0, math.log(r), th, 0.7, u, eps)
+                s2, rho2, Delta = math.sin(th) ** 2, r * r + a * a * math.cos(th) ** 2, r * r - 2 * r + a * a
+                gtt = -((r * r + a * a) ** 2 - a * a * Delta * s2) / (rho2 * Delta)
+                gtp = -2.0 * a * r / (rho2 * Delta)
+                grr, gthth = Delta / rho2, 1.0 / rho2
+                gpp = (Delta - a * a * s2) / (rho2 * Delta * s2)
+                ut = -E
+                norm = gtt * ut * ut + 2 * gtp * ut * u[2] + grr * urb * urb + gthth * u[1] ** 2 + gpp * u[2] ** 2
+                scale = abs(gtt * ut * ut) + grr * urb * urb + gthth * u[1] ** 2 + abs(gpp) * u[2] ** 2 + 1.0
+                assert abs(norm + eps) <= 1e-12 * scale, (a, r, th, eps, norm)
+                assert Gam >= 1.0 - 1e-15 if eps == 1.0 else Gam > 0.0
+        if a > 0:
+            r, h = 3.7, 1e-5
+            d = lambda rr: 0.7 - oracle.ks_to_bl(a, 1.0, math.log(rr), 1.0, 0.7, np.zeros(3))[3]   # phi_KS - phi_BL
+            Delta = r * r - 2 * r + a * a
+            assert abs((d(r + h) - d(r - h)) / (2 * h) - a / Delta) < 1e-8
+        assert abs(oracle.ks_to_bl(a, 1.0, math.log(4.0), 1.1, 0.0, np.zeros(3))[1] - 1.0) < 1e-15
+    # (4) along a Table-1-like bound orbit
+    a = 0.9
+    y0 = np.array([6.0, math.pi / 2, 0.0, 0.05, 0.3, 3.2])
+    traj = oracle.geodesic_traj(a, 1.0, 3, y0, 1e-2, 4000, every=400)
+    Es = [oracle.ks_to_bl(a, 1.0, math.log(y[0]), y[1], y[2], y[3:6])[0] for y in traj]
+    assert max(Es) - min(Es) < 1e-6 * abs(Es[0])
