@@ -170,7 +170,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
-                 "--format=csv,noheader,nounits", "-lms", "50"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
@@ -324,6 +324,7 @@ def run_ours(args):
     cur, alt = grpic.Particles.from_numpy(ptc), grpic.Particles(n)
     n_alive = torch.zeros(W + K + 8, dtype=torch.int64, device="cuda")
     removed = torch.zeros(W + K + 8, dtype=torch.int64, device="cuda")   # lazy removal: particles flagged per step
+    clk = torch.zeros(W + K + 8, 4, dtype=torch.int64, device="cuda")    # SM clock of every push launch (device words)
     stream = torch.cuda.current_stream()
 
     names = ("sort", "push_deposit", "allreduce", "finalize", "field_step", "compact")
@@ -345,6 +346,7 @@ def run_ours(args):
             mark(s, "sort", 1)
             cur, alt = alt, cur
         flux_block.zero_()
+        ctx.set_clock_probe(clk[s])
         mark(s, "push_deposit", 0)
         if fused:       # removal fused into the push: survivors of `cur` are pushed into `alt`
             ctx.push_deposit_compact(cur, alt, fields, flux, dt, n_alive[s:s + 1])
@@ -416,21 +418,27 @@ def run_ours(args):
 
     # ---- sustained FP64 pipe rate (same clocks regime as the long step), then rooflines
     fp64_peak_sust = fp64_peak_burst
+    ctx.set_clock_probe(None)
     tp0 = time.time()
     t_end = tp0 + 1.0
+    c_probe_dev = None
     while time.time() < t_end:
-        fp64_peak_sust = ctx.measure_fp64_peak()
+        fp64_peak_sust, c_probe_dev = ctx.measure_fp64_peak_clocked()
     tp1 = time.time()
     probe_clocks = ClockSampler.summarise(sampler.window(tp0 + 0.5, tp1)) if sampler else None
     if sampler:
         sampler.stop()
+    # SM clock of the timed push launches, measured on the device by the kernel itself
+    cw = clk[W:W + K].cpu().numpy().astype(np.float64)
+    ok = cw[:, 3] > cw[:, 1]
+    push_mhz = 1e3 * (cw[ok, 2] - cw[ok, 0]) / (cw[ok, 3] - cw[ok, 1]) if ok.any() else np.zeros(0)
     # The register-only DFMA probe draws less power than the step (HBM + L2 atomics + FP64): under the
     # board's power cap the timed loop can run at a lower SM clock than the probe.  The pipe's rate is
     # lanes x clock, so the roof the loop is held against is the probe's rate scaled to the loop's clock;
     # the unscaled figure is reported beside it.
     fp64_peak_probe = fp64_peak_sust
-    c_loop = (clocks or {}).get("sm_mhz")
-    c_probe = (probe_clocks or {}).get("sm_mhz")
+    c_loop = float(np.mean(push_mhz)) if len(push_mhz) else (clocks or {}).get("sm_mhz")
+    c_probe = c_probe_dev or (probe_clocks or {}).get("sm_mhz")
     if c_loop and c_probe and c_loop < c_probe:
         fp64_peak_sust = fp64_peak_probe * c_loop / c_probe
     peaks = {}
@@ -464,9 +472,11 @@ def run_ours(args):
                       "source_hash": rc.get("source_hash"), "stale": bool(rc["stale"]),
                       "applies_to_this_run": bool(applies)},
         "stale": bool(rc["stale"]) or not applies,
-        "peak_source": "FP64 DFMA chain measured live on this device after the timed loop, scaled to the "
-                       "SM clock sampled during the timed loop when the power cap held it below the "
-                       "probe's clock; 2 flop per FP64 pipe instruction",
+        "peak_source": "FP64 DFMA chain measured live on this device after the timed loop, scaled to the SM "
+                       "clock of the timed push launches (cycle counter / nanosecond timer, read by the kernels "
+                       "themselves) when the power cap held it below the probe's clock; 2 flop per FP64 pipe "
+                       "instruction.  frac_at_probe_clock is the unscaled figure",
+        "sm_mhz_per_push": [round(float(x), 1) for x in push_mhz],
         "peak_probe": 2.0 * fp64_peak_probe / 1e12, "sm_mhz_loop": c_loop, "sm_mhz_probe": c_probe,
         "frac_at_probe_clock": fp64_pp * per_launch / fp64_peak_probe / (pd_ms * 1e-3),
         "peak_burst": 2.0 * fp64_peak_burst / 1e12,

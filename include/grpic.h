@@ -257,10 +257,19 @@ int grpic_deposit_rho(grpic_ctx* ctx, const grpic_particles* ptc, double* rho, i
 int grpic_ks_to_bl(grpic_ctx* ctx, const grpic_particles* ptc, double* E_inf, double* gamma_fido,
                    double* ur_bl, double* phi_bl, void* stream);
 
+/* Measurement aid: the SM clock a push ran at.  When set, every grpic_push_deposit(_compact) launch
+ * writes four DEVICE words { cycle counter at start, nanosecond timer at start, cycle counter at the
+ * end, nanosecond timer at the end } taken by the first thread of its persistent grid; (w[2]-w[0]) /
+ * (w[3]-w[1]) is the SM clock in GHz during that launch (under the board's power cap it can be lower
+ * than the clock of a register-only probe kernel).  NULL (the default) disables it. */
+int grpic_set_clock_probe(grpic_ctx* ctx, unsigned long long* device_words4);
+
 /* Roofline denominator: measured FP64 pipe throughput of this device.  Runs a register-only
  * kernel of independent DFMA chains on every SM (blocking, ~10 ms) and writes the achieved
  * FP64 instructions (lane-operations) per second to the HOST double *dfma_per_second. */
 int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second);
+/* The same, also returning the SM clock (MHz, cycle counter over nanosecond timer) the probe ran at. */
+int grpic_measure_fp64_peak_clocked(grpic_ctx* ctx, double* dfma_per_second, double* sm_mhz);
 
 /* Number of CUDA kernels this library has launched in this process so far (all contexts);
  * used by bench.py to report `gpu_launches`. */

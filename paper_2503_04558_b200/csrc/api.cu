@@ -104,7 +104,14 @@ __global__ void areas_kernel(GridDev g, double* ADr, double* ADth, double* ADph,
 }
 
 // FP64 pipe microbenchmark: 8 independent DFMA chains per thread, registers only.
-__global__ void __launch_bounds__(256) dfma_kernel(double* out, int iters, double seed) {
+__global__ void __launch_bounds__(256) dfma_kernel(double* out, int iters, double seed, unsigned long long* clk) {
+  const bool probe = clk && blockIdx.x == 0 && threadIdx.x == 0;
+  if (probe) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    clk[0] = (unsigned long long)clock64();
+    clk[1] = t;
+  }
   double x0 = seed + threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5,
          x6 = x0 + 6, x7 = x0 + 7;
   const double m = 0.999999, b = 1e-9;
@@ -117,6 +124,12 @@ __global__ void __launch_bounds__(256) dfma_kernel(double* out, int iters, doubl
   }
   const double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
   if (s == 123.456) out[0] = s;   // never true; keeps the chains alive
+  if (probe) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    clk[2] = (unsigned long long)clock64();
+    clk[3] = t;
+  }
 }
 
 int launch_areas(const GridDev& g, double* const out[6], int factors, cudaStream_t st) {
@@ -150,6 +163,7 @@ int grpic_create(const grpic_params* p, grpic_ctx** out) {
   ctx->ws_bytes = 0;
   ctx->host_step = nullptr;
   ctx->removed_counter = nullptr;
+  ctx->clock_probe = nullptr;
   ctx->flux_exchange = nullptr;
   ctx->flux_exchange_user = nullptr;
   cudaDeviceGetAttribute(&ctx->sm_count, cudaDevAttrMultiProcessorCount, dev);
@@ -245,6 +259,12 @@ int grpic_set_removed_counter(grpic_ctx* ctx, unsigned long long* device_counter
   return GRPIC_OK;
 }
 
+int grpic_set_clock_probe(grpic_ctx* ctx, unsigned long long* device_words4) {
+  if (!ctx) return GRPIC_ERR_ARG;
+  ctx->clock_probe = device_words4;
+  return GRPIC_OK;
+}
+
 int grpic_set_flux_exchange(grpic_ctx* ctx, grpic_flux_exchange_fn fn, void* user) {
   if (!ctx) return GRPIC_ERR_ARG;
   ctx->flux_exchange = fn;
@@ -261,7 +281,13 @@ int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes) {
 }
 
 int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second) {
+  return grpic_measure_fp64_peak_clocked(ctx, dfma_per_second, nullptr);
+}
+
+int grpic_measure_fp64_peak_clocked(grpic_ctx* ctx, double* dfma_per_second, double* sm_mhz) {
   if (!ctx || !dfma_per_second) return GRPIC_ERR_ARG;
+  unsigned long long* clk = nullptr;
+  if (sm_mhz && cudaMalloc(&clk, 4 * sizeof(unsigned long long)) != cudaSuccess) return GRPIC_ERR_ALLOC;
   const int iters = 4096, blocks = ctx->sm_count * 8;
   cudaEvent_t e0, e1;
   GRPIC_CUDA_OK(cudaEventCreate(&e0));
@@ -269,7 +295,7 @@ int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second) {
   double best = 0.0;
   for (int rep = 0; rep < 4; ++rep) {
     cudaEventRecord(e0, 0);
-    dfma_kernel<<<blocks, 256>>>(ctx->tables, iters, 1.0);
+    dfma_kernel<<<blocks, 256>>>(ctx->tables, iters, 1.0, clk);
     cudaEventRecord(e1, 0);
     if (cudaEventSynchronize(e1) != cudaSuccess) return GRPIC_ERR_CUDA;
     float ms = 0.f;
@@ -281,6 +307,12 @@ int grpic_measure_fp64_peak(grpic_ctx* ctx, double* dfma_per_second) {
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   *dfma_per_second = best;
+  if (clk) {                                          // SM clock of the last repetition: cycles / nanoseconds
+    unsigned long long h[4] = {0, 0, 0, 1};
+    cudaMemcpy(h, clk, sizeof(h), cudaMemcpyDeviceToHost);
+    cudaFree(clk);
+    *sm_mhz = h[3] > h[1] ? 1e3 * (double)(h[2] - h[0]) / (double)(h[3] - h[1]) : 0.0;
+  }
   return grpic_launch_ok();
 }
 

@@ -38,6 +38,7 @@ struct grpic_ctx {
   size_t ws_bytes;
   int sm_count;
   unsigned long long* removed_counter;   // grpic_set_removed_counter (caller's device word, nullable)
+  unsigned long long* clock_probe;       // grpic_set_clock_probe (caller's 4 device words, nullable)
   grpic_flux_exchange_fn flux_exchange;  // grpic_set_flux_exchange (multi-GPU sum of the fluxes in grpic_step_host)
   void* flux_exchange_user;
   void* host_step;  // staging buffers / streams of grpic_step_host (host_step.cu), lazily created

@@ -169,13 +169,25 @@ constexpr uint32_t kTileBytes = 7u * kWTile * 8u + kWTile * 4u;
 // live lanes (offsets = exclusive scan of the per-tile live counts of `ptc`), i.e. particles
 // already flagged removed are squeezed out on the way, order preserved; the weight travels along.
 // Otherwise dst == ptc and the update is in place.
+// registers per thread for MINB resident 64-thread CTAs: 8 -> 128, 9 -> 112, 10 -> 96 (ptxas left to
+// itself picks 96 for MINB = 9)
+constexpr int pd_max_regs(int minb) { return minb <= 8 ? 128 : (minb == 9 ? 112 : 96); }
 template <int MINB, bool COMPACT, int KT, bool TAB>
-__global__ void __launch_bounds__(kBlock, MINB)
+__global__ void __launch_bounds__(kBlock) __maxnreg__(pd_max_regs(MINB))
 push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
                     const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
                     const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
                     const __grid_constant__ PolyTab pt, double dt, int K, uint32_t* status,
-                    unsigned long long* removed) {
+                    unsigned long long* removed, unsigned long long* clock_probe) {
+  // SM clock during this launch (grpic_set_clock_probe): the first thread of the persistent grid notes
+  // the SM cycle counter and the nanosecond timer when it starts and when it has pushed its last tile
+  const bool probe = clock_probe && blockIdx.x == 0 && threadIdx.x == 0;
+  if (probe) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    clock_probe[0] = (unsigned long long)clock64();
+    clock_probe[1] = t;
+  }
   __shared__ WTile tiles[kWarps][kPdStages];
   __shared__ __align__(8) uint64_t full[kWarps][kPdStages];
   // COMPACT: the aligned 16 bytes of `offsets` that hold each staged tile's two output offsets.
@@ -453,6 +465,12 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     tile += wstride;
   }
   }
+  if (probe) {
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    clock_probe[2] = (unsigned long long)clock64();
+    clock_probe[3] = t;
+  }
 }
 
 template <int MINB, bool COMPACT, int KT, bool TAB>
@@ -469,7 +487,8 @@ int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const 
   const int64_t resident = (int64_t)ctx->sm_count * per_sm;
   const unsigned grid = (unsigned)(nblocks < resident ? nblocks : resident);
   push_deposit_kernel<MINB, COMPACT, KT, TAB><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, f, J, kPolyTabHost, dt,
-                                                                  ctx->p.geo_iters, status, ctx->removed_counter);
+                                                                  ctx->p.geo_iters, status, ctx->removed_counter,
+                                                                  ctx->clock_probe);
   return grpic_launch_ok();
 }
 

@@ -50,7 +50,7 @@ EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_area
            "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
            "grpic_circulation", "grpic_ks_to_bl", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
-           "grpic_measure_fp64_peak", "grpic_kernel_launches", "grpic_strerror"]
+           "grpic_measure_fp64_peak", "grpic_measure_fp64_peak_clocked", "grpic_set_clock_probe", "grpic_kernel_launches", "grpic_strerror"]
 
 _lib = None
 
@@ -357,6 +357,17 @@ class Context:
         ps = ptc.struct()
         _check(load().grpic_ks_to_bl(self.h, C.byref(ps), *[_ptr(t) for t in out], _stream()))
         return [t[:ptc.n] for t in out]
+
+    def set_clock_probe(self, words):
+        """words: int64 device tensor of 4 elements (or None), see grpic_set_clock_probe"""
+        self._clk = words
+        _check(load().grpic_set_clock_probe(self.h, C.c_void_p(words.data_ptr()) if words is not None else None))
+
+    def measure_fp64_peak_clocked(self):
+        """(FP64 instructions per second, SM clock in MHz during the probe)"""
+        v, c = C.c_double(0.0), C.c_double(0.0)
+        _check(load().grpic_measure_fp64_peak_clocked(self.h, C.byref(v), C.byref(c)))
+        return v.value, c.value
 
     def measure_fp64_peak(self):
         """measured FP64 pipe rate of this device, FP64 instructions (lane-ops) per second"""
