@@ -38,6 +38,12 @@ namespace {
 #define GRPIC_PD_MB 10     // 96 registers per thread: the in-place variant
 #endif
 constexpr int kBlock = GRPIC_PD_BLOCK;
+// Ablation switches for the cost table in profiles/ (NOT for production: they change the result).
+// Build with e.g. GRPIC_NVCC_EXTRA="-DGRPIC_ABL_NO_DEPOSIT" python -m paper_2503_04558_b200.build --force
+//   GRPIC_ABL_NO_GATHER   the 24 field loads are replaced by values made from the position
+//   GRPIC_ABL_NO_BORIS    the Boris step is skipped
+//   GRPIC_ABL_NO_DEPOSIT  no REDs (the deposit arithmetic goes with them)
+//   GRPIC_ABL_K=<n>       n corrector iterations instead of the context's K (0..3)
 
 // Charge-conserving deposit of one move (Eq.21-23) on the 3x3-node window anchored at the
 // lower of the old and new cell in each direction: a move of less than one cell touches at
@@ -305,10 +311,15 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       const uint32_t b6[6] = {bhn, bnh, bnn, bnh, bhn, bhh};
 #pragma unroll
       for (int c = 0; c < 6; ++c) {
+#ifdef GRPIC_ABL_NO_GATHER
+        G[c][0] = x1 * (c + 1); G[c][1] = x2 + c; G[c][2] = x1 - c; G[c][3] = x2 * (c + 2);
+        (void)F6; (void)b6;
+#else
         G[c][0] = __ldg(F6[c] + b6[c]);
         G[c][1] = __ldg(F6[c] + b6[c] + 1);
         G[c][2] = __ldg(F6[c] + b6[c] + g.pitch);
         G[c][3] = __ldg(F6[c] + b6[c] + g.pitch + 1);
+#endif
       }
     }
 
@@ -350,7 +361,11 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
 
     // ---- Boris (full dt) at x^n ----
     double ur = T.u1[sl], ut = T.u2[sl], up = T.u3[sl];
+#ifndef GRPIC_ABL_NO_BORIS
     boris(g, p0, alpha0, sgn, dt, D, B, ur, ut, up);
+#else
+    ur += 1e-300 * (D[0] + D[1] + D[2] + B[0] + B[1] + B[2]);     // keeps the gather alive
+#endif
 
     // ---- geodesic predictor + K correctors (Eq.14, 15) ----
     double Xr0, Xt0, Xp0, Ur0, Ut0;
@@ -358,7 +373,12 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     double dr = Xr0 * dt, dth = Xt0 * dt, dph = Xp0 * dt;      // increments from x^n
     double vr = fma(Ur0, dt, ur), vt = fma(Ut0, dt, ut);
     const double hdt = 0.5 * dt;
+#ifdef GRPIC_ABL_K
+    const int KK = GRPIC_ABL_K;
+    (void)K;
+#else
     const int KK = KT > 0 ? KT : K;                 // KT: compile-time corrector count (unrolled)
+#endif
 #pragma unroll
     for (int ci = 0; ci < KK; ++ci) {
       double s, c;
@@ -445,7 +465,11 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     __stcs(dst.flag + kd, nflag);
 
     // ---- deposit: 3x3 window anchored at the lower of the old / new cell ----
+#ifdef GRPIC_ABL_NO_DEPOSIT
+    if (false) {
+#else
     if (finite && !photon && !offgrid) {
+#endif
       const double q = sgn * T.w[sl];
       const double vph = q * dph * idt;
       const int di = ib - ia, dj = jb - ja;
