@@ -508,7 +508,12 @@ def run_ours(args):
         sb = 176.0 * n / 1e9
         ms = phases["sort"]["ms_per_call"]
         kernels["sort"] = {"ms": ms, "bound": "hbm", "achieved": sb / (ms * 1e-3), "peak": hbm_peak,
-                           "unit": "GB/s", "frac": sb / (ms * 1e-3) / hbm_peak}
+                           "unit": "GB/s", "frac": sb / (ms * 1e-3) / hbm_peak,
+                           "state": "steady state: the input is the order of the previous sort, %d steps old" % sort_every}
+        if (0, "sort", 0) in ev and W > 0:      # the very first sort (warm-up step 0): randomly ordered input
+            ms0 = ev[(0, "sort", 0)].elapsed_time(ev[(0, "sort", 1)])
+            kernels["sort"]["first_unsorted_ms"] = ms0
+            kernels["sort"]["first_unsorted_frac"] = sb / (ms0 * 1e-3) / hbm_peak
     if "compact" in phases:
         cb = 132.0 * n / 1e9
         ms = phases["compact"]["ms_per_call"]
