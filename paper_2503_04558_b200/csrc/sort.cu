@@ -2,6 +2,8 @@
 // of removed particles, with warp-level match/ballot ranking.  Hand-written for sm_100a; no
 // CUB/Thrust.  Sort is not part of the paper (BASELINE.json north_star); removal follows
 // PAPER.md:138,:364.
+#include <stdlib.h>
+
 #include "grpic_internal.cuh"
 
 namespace {
@@ -109,19 +111,28 @@ radix_hist_kernel(const uint32_t* keys, const uint32_t* cell, const uint32_t* fl
   hist[(size_t)threadIdx.x * ntiles + blockIdx.x] = sh[threadIdx.x];
 }
 
-// stable scatter of one tile: warp w owns keys [w*256, w*256+256) of the tile in 8 groups
+// stable scatter of one tile: warp w owns keys [w*256, w*256+256) of the tile in 8 groups.
+// The tile is first sorted by digit in shared memory (position = exclusive prefix of the tile's digit
+// counts + stable rank of the key among the tile's keys of that digit), then written out in that
+// order: all keys of one digit go to consecutive global positions, so every warp store covers whole
+// runs instead of 32 scattered 4-byte elements (pass 1 at 1e8 keys: 1.08 -> see profiles/r02_final.md).
 template <bool FIRST>
 __global__ void __launch_bounds__(kThreads)
 radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint32_t* cell,
                      const uint32_t* flag, int64_t n, uint32_t ncells, int shift,
                      const uint32_t* hist_scanned, uint32_t ntiles, uint32_t* keys_out,
                      uint32_t* idx_out) {
-  __shared__ uint32_t whist[kThreads / 32][kRadix];
+  __shared__ uint32_t whist[kThreads / 32][kRadix];   // per-warp digit counts, then local starts
+  __shared__ uint32_t tstart[kRadix];                  // exclusive prefix of the tile's digit counts
+  __shared__ uint32_t gstart[kRadix];                  // global start of the tile's run of each digit
+  __shared__ uint32_t skey[kTile], sidx[kTile];
+  __shared__ uint32_t wsum[kThreads / 32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
 #pragma unroll
   for (int q = 0; q < kThreads / 32; ++q) whist[q][threadIdx.x] = 0;
   __syncthreads();
-  const int64_t wbase = (int64_t)blockIdx.x * kTile + (int64_t)w * (kGroups * 32);
+  const int64_t tbase = (int64_t)blockIdx.x * kTile;
+  const int64_t wbase = tbase + (int64_t)w * (kGroups * 32);
   uint32_t key[kGroups], idx[kGroups], dig[kGroups];
 #pragma unroll
   for (int q = 0; q < kGroups; ++q) {
@@ -142,9 +153,25 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
     __syncwarp();
   }
   __syncthreads();
-  // 2. digit t: global start of each warp's run = scanned histogram + counts of earlier warps
+  // 2. thread d: tile count of digit d, exclusive prefix over the digits (block scan), local start
+  //    of every warp's run inside the tile's sorted order, global start of the tile's run
   {
-    uint32_t run = hist_scanned[(size_t)threadIdx.x * ntiles + blockIdx.x];
+    uint32_t tot = 0;
+#pragma unroll
+    for (int q = 0; q < kThreads / 32; ++q) tot += whist[q][threadIdx.x];
+    uint32_t incl = tot;
+#pragma unroll
+    for (int d = 1; d < 32; d <<= 1) {
+      const uint32_t t = __shfl_up_sync(0xffffffffu, incl, d);
+      if (lane >= d) incl += t;
+    }
+    if (lane == 31) wsum[w] = incl;
+    __syncthreads();
+    uint32_t off = 0;
+    for (int q = 0; q < w; ++q) off += wsum[q];
+    uint32_t run = off + incl - tot;                 // exclusive prefix of digit threadIdx.x
+    tstart[threadIdx.x] = run;
+    gstart[threadIdx.x] = hist_scanned[(size_t)threadIdx.x * ntiles + blockIdx.x];
 #pragma unroll
     for (int q = 0; q < kThreads / 32; ++q) {
       const uint32_t cnt = whist[q][threadIdx.x];
@@ -153,7 +180,8 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
     }
   }
   __syncthreads();
-  // 3. rank inside the warp, group by group (keeps the input order of equal digits)
+  // 3. rank inside the warp, group by group (keeps the input order of equal digits): position in
+  //    the tile's sorted order
   const uint32_t lt = (1u << lane) - 1u;
 #pragma unroll
   for (int q = 0; q < kGroups; ++q) {
@@ -164,8 +192,21 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
     if (dig[q] < kRadix && lane == (__ffs(peers) - 1)) whist[w][dig[q]] += __popc(peers);
     __syncwarp();
     if (dig[q] < kRadix) {
-      keys_out[pos] = key[q];
-      idx_out[pos] = idx[q];
+      skey[pos] = key[q];
+      sidx[pos] = idx[q];
+    }
+  }
+  __syncthreads();
+  // 4. write the tile in sorted order: element e of the tile goes to gstart[d] + (e - tstart[d])
+  const uint32_t cnt_tile = (uint32_t)((n - tbase) < (int64_t)kTile ? (n - tbase) : (int64_t)kTile);
+#pragma unroll
+  for (int m = 0; m < kTile / kThreads; ++m) {
+    const uint32_t e = m * kThreads + threadIdx.x;
+    if (e < cnt_tile) {
+      const uint32_t k = skey[e], d = (k >> shift) & 0xFFu;
+      const uint32_t pos = gstart[d] + (e - tstart[d]);
+      keys_out[pos] = k;
+      idx_out[pos] = sidx[e];
     }
   }
 }
@@ -354,6 +395,8 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, u
     grpic_count_launches(2);
   }
   if (interleave) {
+    // (moving the payload inside the rank loop instead of writing perm2 first was measured: 24.7 ms
+    // against 6.7 ms -- the loop is latency-bound, the separate gather runs at 4.6 TB/s)
     cell_start_kernel<<<(ncells + 2 + 255) / 256, 256, 0, st>>>(kin, (uint32_t)n, ncells, start);
     interleave_perm_kernel<<<(ncells + 255) / 256, 256, 0, st>>>(iin, start, (uint32_t)n, ncells, (uint32_t)interleave, iout);
     uint32_t* t = iin; iin = iout; iout = t;
