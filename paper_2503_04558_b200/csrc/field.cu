@@ -89,6 +89,12 @@ __device__ __forceinline__ void tma_load_1d(void* dst, const void* src, uint32_t
       "l"(src), "r"(bytes), "r"(smem_u32(bar))
       : "memory");
 }
+// one lane of the (converged) warp: the guarded region stays on the uniform datapath
+__device__ __forceinline__ bool elect_one() {
+  uint32_t p;
+  asm volatile("{ .reg .pred P; elect.sync _|P, 0xffffffff; selp.u32 %0, 1, 0, P; }" : "=r"(p));
+  return p != 0;
+}
 __device__ __forceinline__ void prefetch_l1(const double* p) {
   asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 }
@@ -133,24 +139,34 @@ template <int MODE, bool FAST, bool TMA>
 __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A, int lane, int ibase,
                                            int jstart, int jend, double* ring, uint64_t* bars) {
   const int i = ibase - 2 + lane;                       // this lane's column
-  // ---- TMA plumbing: this lane's source array and row offset inside a packet ----
-  const double* myptr = nullptr;
-  if (TMA) {
-    const double* const areas[6] = {g.iADr, g.iADth, g.iADph, g.iABr, g.iABth, g.iABph};
-    if (lane < 6) myptr = A.in[lane];
-    else if (lane < 12) myptr = (MODE != 2) ? A.base[lane - 6] : nullptr;
-    else if (lane < kSeg) myptr = areas[lane - 12];
-  }
+  // ---- TMA plumbing.  One elected lane arms the stage's mbarrier and issues the packet's 18 (6 in the
+  // first iteration, 12 for the diagnostics mode) bulk copies with warp-uniform addresses.  (Round 1
+  // let lanes 0..17 issue one copy each: ptxas serialises such divergent UBLKCP issue in an
+  // ELECT / R2UR / BRA.U loop, ~160 of the 613 instructions per row, profiles/r02_final.md.) ----
   auto request = [&](int jj, int stage) {               // packet jj -> ring stage
     if (jj > jend) return;
     const bool epi = (jj - 1 >= jstart);                // epilogue operands of row jj-1 wanted
-    const uint32_t nseg = epi ? (MODE != 2 ? 18u : 12u) : 6u;
-    if (lane == 0) mbar_expect_tx(&bars[stage], nseg * 256u);
-    __syncwarp();
-    const bool mine = (lane < 6) || (epi && lane < kSeg && myptr != nullptr);
-    if (mine) {
-      const size_t k0 = g.idx(ibase - 2, lane < 6 ? jj : jj - 1);
-      tma_load_1d(ring + (stage * kSeg + lane) * 32, myptr + k0, 256u, &bars[stage]);
+    if (elect_one()) {
+      const uint32_t nseg = epi ? (MODE != 2 ? 18u : 12u) : 6u;
+      uint64_t* bar = &bars[stage];
+      double* dst = ring + stage * kSeg * 32;
+      mbar_expect_tx(bar, nseg * 256u);
+      const size_t k0 = g.idx(ibase - 2, jj);
+#pragma unroll
+      for (int c = 0; c < 6; ++c) tma_load_1d(dst + c * 32, A.in[c] + k0, 256u, bar);
+      if (epi) {
+        const size_t k1 = k0 - (size_t)g.pitch;
+        if (MODE != 2) {
+#pragma unroll
+          for (int c = 0; c < 6; ++c) tma_load_1d(dst + (6 + c) * 32, A.base[c] + k1, 256u, bar);
+        }
+        tma_load_1d(dst + 12 * 32, g.iADr + k1, 256u, bar);
+        tma_load_1d(dst + 13 * 32, g.iADth + k1, 256u, bar);
+        tma_load_1d(dst + 14 * 32, g.iADph + k1, 256u, bar);
+        tma_load_1d(dst + 15 * 32, g.iABr + k1, 256u, bar);
+        tma_load_1d(dst + 16 * 32, g.iABth + k1, 256u, bar);
+        tma_load_1d(dst + 17 * 32, g.iABph + k1, 256u, bar);
+      }
     }
   };
   if (TMA) {
@@ -316,14 +332,14 @@ field_sweep_kernel(const __grid_constant__ GridDev g, const __grid_constant__ Sw
     else if (id < edge + axis) { bx = 1 + (id - edge) % ic; by = ((id - edge) / ic) ? A.nchunks - 1 : 0; }
     else { bx = 1 + (id - edge - axis) % ic; by = 1 + (id - edge - axis) / ic; }
   }
-  const int wcol = bx * kWarpsPerBlock + (threadIdx.x >> 5);
+  const int w = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);   // provably warp-uniform
+  const int wcol = bx * kWarpsPerBlock + w;
   const int ibase = wcol * kOutCols;
   if (ibase > g.nr) return;
   const int jstart = by * A.row_chunk;
   const int jend = min(jstart + A.row_chunk, g.nth + 1);  // output rows [jstart, jend)
   __shared__ __align__(128) double ring[kWarpsPerBlock][kStages * kSeg * 32];
   __shared__ __align__(8) uint64_t bars[kWarpsPerBlock][kStages];
-  const int w = threadIdx.x >> 5;
   const bool fast = (ibase >= 1) && (ibase + kOutCols - 1 <= g.nr - 2) && (jstart >= 1) && (jend <= g.nth);
   if (fast && A.tma) sweep_rows<MODE, true, true>(g, A, lane, ibase, jstart, jend, ring[w], bars[w]);
   else if (fast) sweep_rows<MODE, true, false>(g, A, lane, ibase, jstart, jend, nullptr, nullptr);
