@@ -143,6 +143,16 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
   // first iteration, 12 for the diagnostics mode) bulk copies with warp-uniform addresses.  (Round 1
   // let lanes 0..17 issue one copy each: ptxas serialises such divergent UBLKCP issue in an
   // ELECT / R2UR / BRA.U loop, ~160 of the 613 instructions per row, profiles/r02_final.md.) ----
+  // the 18 source addresses of the warp's column strip at row 0, kept across the row loop (uniform
+  // registers): a request adds the row offset, nothing else
+  const double* src[kSeg];
+  if (TMA) {
+    const size_t kb = g.idx(ibase - 2, 0);
+#pragma unroll
+    for (int c = 0; c < 6; ++c) { src[c] = A.in[c] + kb; src[6 + c] = (MODE != 2) ? A.base[c] + kb : nullptr; }
+    src[12] = g.iADr + kb; src[13] = g.iADth + kb; src[14] = g.iADph + kb;
+    src[15] = g.iABr + kb; src[16] = g.iABth + kb; src[17] = g.iABph + kb;
+  }
   auto request = [&](int jj, int stage) {               // packet jj -> ring stage
     if (jj > jend) return;
     const bool epi = (jj - 1 >= jstart);                // epilogue operands of row jj-1 wanted
@@ -151,21 +161,12 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
       uint64_t* bar = &bars[stage];
       double* dst = ring + stage * kSeg * 32;
       mbar_expect_tx(bar, nseg * 256u);
-      const size_t k0 = g.idx(ibase - 2, jj);
+      const ptrdiff_t r0 = (ptrdiff_t)jj * g.pitch, r1 = r0 - g.pitch;
 #pragma unroll
-      for (int c = 0; c < 6; ++c) tma_load_1d(dst + c * 32, A.in[c] + k0, 256u, bar);
+      for (int c = 0; c < 6; ++c) tma_load_1d(dst + c * 32, src[c] + r0, 256u, bar);
       if (epi) {
-        const size_t k1 = k0 - (size_t)g.pitch;
-        if (MODE != 2) {
 #pragma unroll
-          for (int c = 0; c < 6; ++c) tma_load_1d(dst + (6 + c) * 32, A.base[c] + k1, 256u, bar);
-        }
-        tma_load_1d(dst + 12 * 32, g.iADr + k1, 256u, bar);
-        tma_load_1d(dst + 13 * 32, g.iADth + k1, 256u, bar);
-        tma_load_1d(dst + 14 * 32, g.iADph + k1, 256u, bar);
-        tma_load_1d(dst + 15 * 32, g.iABr + k1, 256u, bar);
-        tma_load_1d(dst + 16 * 32, g.iABth + k1, 256u, bar);
-        tma_load_1d(dst + 17 * 32, g.iABph + k1, 256u, bar);
+        for (int c = (MODE != 2 ? 6 : 12); c < kSeg; ++c) tma_load_1d(dst + c * 32, src[c] + r1, 256u, bar);
       }
     }
   };
