@@ -410,8 +410,10 @@ int launch_sweep(const grpic_ctx* ctx, SweepArgs A, cudaStream_t st) {
   const GridDev& g = ctx->g;
   const int wcols = (g.nr + 1 + kOutCols - 1) / kOutCols;
   const int bcols = (wcols + kWarpsPerBlock - 1) / kWarpsPerBlock;
-  // rows per warp: as many row chunks per column block as fill the resident CTAs exactly once
-  // (one full wave, every warp the same work), but at least 16 rows (2 halo rows per chunk)
+  // rows per warp: whole waves of the resident CTAs, at most max_rows rows per chunk (2 halo rows
+  // per chunk), at least 8.  Measured after the TMA issue went to one elected lane (field step at
+  // 2048^2 / 4096^2, ms): cap 8: 1.363 / 5.02, 12: 1.359 / 5.00, 16: 1.353 / 4.90, 20: 1.351 / 4.87,
+  // 32: 1.428 / 4.93, 48: 1.735 (longer chunks lose DRAM page locality and leave fewer CTAs per wave)
   static int per_sm = 0;
   if (per_sm == 0) {
     if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, field_sweep_kernel<MODE>, 32 * kWarpsPerBlock,
@@ -419,7 +421,7 @@ int launch_sweep(const grpic_ctx* ctx, SweepArgs A, cudaStream_t st) {
       per_sm = 1;
   }
   static int max_rows = -1;
-  if (max_rows < 0) { const char* e = getenv("GRPIC_FS_MAXROWS"); max_rows = e ? atoi(e) : 32; }
+  if (max_rows < 0) { const char* e = getenv("GRPIC_FS_MAXROWS"); max_rows = e ? atoi(e) : 20; }
   const int resident = ctx->sm_count * per_sm;
   const int nrows = g.nth + 1;
   const int min_chunks = (nrows + max_rows - 1) / max_rows;
@@ -427,7 +429,7 @@ int launch_sweep(const grpic_ctx* ctx, SweepArgs A, cudaStream_t st) {
   int chunks = waves * resident / bcols;
   if (chunks < min_chunks) chunks = min_chunks;
   int rows = (nrows + chunks - 1) / chunks;
-  if (rows < 16) rows = 16;
+  if (rows < 8) rows = 8;
   A.row_chunk = rows;
   A.bcols = bcols;
   A.nchunks = (g.nth + 1 + rows - 1) / rows;
