@@ -95,6 +95,13 @@ __device__ __forceinline__ bool elect_one() {
   asm volatile("{ .reg .pred P; elect.sync _|P, 0xffffffff; selp.u32 %0, 1, 0, P; }" : "=r"(p));
   return p != 0;
 }
+// 256-byte bulk copy global -> shared from raw addresses (shared-window destination and barrier)
+__device__ __forceinline__ void tma_load_raw(uint32_t dst32, uint64_t src, uint32_t bar32) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], 256, [%2];" ::"r"(dst32),
+      "l"(src), "r"(bar32)
+      : "memory");
+}
 __device__ __forceinline__ void prefetch_l1(const double* p) {
   asm volatile("prefetch.global.L1 [%0];" ::"l"(p));
 }
@@ -143,30 +150,31 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
   // first iteration, 12 for the diagnostics mode) bulk copies with warp-uniform addresses.  (Round 1
   // let lanes 0..17 issue one copy each: ptxas serialises such divergent UBLKCP issue in an
   // ELECT / R2UR / BRA.U loop, ~160 of the 613 instructions per row, profiles/r02_final.md.) ----
-  // the 18 source addresses of the warp's column strip at row 0, kept across the row loop (uniform
-  // registers): a request adds the row offset, nothing else
-  const double* src[kSeg];
-  if (TMA) {
-    const size_t kb = g.idx(ibase - 2, 0);
-#pragma unroll
-    for (int c = 0; c < 6; ++c) { src[c] = A.in[c] + kb; src[6 + c] = (MODE != 2) ? A.base[c] + kb : nullptr; }
-    src[12] = g.iADr + kb; src[13] = g.iADth + kb; src[14] = g.iADph + kb;
-    src[15] = g.iABr + kb; src[16] = g.iABth + kb; src[17] = g.iABph + kb;
-  }
   auto request = [&](int jj, int stage) {               // packet jj -> ring stage
     if (jj > jend) return;
     const bool epi = (jj - 1 >= jstart);                // epilogue operands of row jj-1 wanted
     if (elect_one()) {
       const uint32_t nseg = epi ? (MODE != 2 ? 18u : 12u) : 6u;
-      uint64_t* bar = &bars[stage];
-      double* dst = ring + stage * kSeg * 32;
-      mbar_expect_tx(bar, nseg * 256u);
-      const ptrdiff_t r0 = (ptrdiff_t)jj * g.pitch, r1 = r0 - g.pitch;
+      const uint32_t bar32 = smem_u32(&bars[stage]);
+      const uint32_t dst32 = smem_u32(ring) + (uint32_t)stage * (kSeg * 256u);
+      mbar_expect_tx(&bars[stage], nseg * 256u);
+      // one byte offset for the six iterate rows (row jj), one for the epilogue operands (row jj-1):
+      // every copy is then pointer + offset
+      const uint64_t off0 = ((uint64_t)(jj + g.j0) * (uint64_t)g.pitch + (uint64_t)(ibase - 2 + g.i0)) * 8u;
+      const uint64_t off1 = off0 - (uint64_t)g.pitch * 8u;
 #pragma unroll
-      for (int c = 0; c < 6; ++c) tma_load_1d(dst + c * 32, src[c] + r0, 256u, bar);
+      for (int c = 0; c < 6; ++c) tma_load_raw(dst32 + c * 256u, (uint64_t)A.in[c] + off0, bar32);
       if (epi) {
+        if (MODE != 2) {
 #pragma unroll
-        for (int c = (MODE != 2 ? 6 : 12); c < kSeg; ++c) tma_load_1d(dst + c * 32, src[c] + r1, 256u, bar);
+          for (int c = 0; c < 6; ++c) tma_load_raw(dst32 + (6 + c) * 256u, (uint64_t)A.base[c] + off1, bar32);
+        }
+        tma_load_raw(dst32 + 12 * 256u, (uint64_t)g.iADr + off1, bar32);
+        tma_load_raw(dst32 + 13 * 256u, (uint64_t)g.iADth + off1, bar32);
+        tma_load_raw(dst32 + 14 * 256u, (uint64_t)g.iADph + off1, bar32);
+        tma_load_raw(dst32 + 15 * 256u, (uint64_t)g.iABr + off1, bar32);
+        tma_load_raw(dst32 + 16 * 256u, (uint64_t)g.iABth + off1, bar32);
+        tma_load_raw(dst32 + 17 * 256u, (uint64_t)g.iABph + off1, bar32);
       }
     }
   };
