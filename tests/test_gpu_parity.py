@@ -1301,3 +1301,36 @@ def test_vacuum_wald_relaxation_quantitative(G, O):
     assert h1 < h0 / 50.0
     assert abs(flux1 - fw) < 0.1 * fw and flux1 < 0.1 * flux0
     assert errs[0][0] < 5e-3 and errs[1][0] < 2e-2
+
+
+def test_clock_probe_and_removed_counter(G, O):
+    """grpic_set_clock_probe: a push launch reports start / end SM cycle counter and nanosecond timer
+    (plausible clock, positive duration); grpic_set_removed_counter: += the number of particles the
+    launch flagged removed, equal to the oracle's count, for the in-place and the compacting push."""
+    cfg = small_case(3, 80, 72, 40000)
+    p, dt, fields, ptc = cfg["params"], cfg["dt"], cfg["fields"], cfg["particles"]
+    ref = O.push(p, fields, ptc, dt)
+    n_gone = int(((ref["flag"] & 2) != 0).sum())
+    assert n_gone > 0
+    ctx = G.Context(p, len(ptc["x1"]))
+    f_t = [ctx.to_device(f) for f in fields]
+    words = torch.zeros(4, dtype=torch.int64, device="cuda")
+    cnt = torch.zeros(2, dtype=torch.int64, device="cuda")
+    P = G.Particles.from_numpy(ptc)
+    ctx.set_clock_probe(words)
+    ctx.set_removed_counter(cnt[0:1])
+    ctx.push_deposit(P, f_t, ctx.zeros(3), dt)
+    torch.cuda.synchronize()
+    w = words.cpu().numpy()
+    assert w[3] > w[1] and w[2] > w[0]
+    mhz = 1e3 * float(w[2] - w[0]) / float(w[3] - w[1])
+    assert 300.0 < mhz < 3000.0, mhz
+    A, B = G.Particles.from_numpy(ptc), G.Particles(len(ptc["x1"]))
+    na = torch.zeros(1, dtype=torch.int64, device="cuda")
+    ctx.set_removed_counter(cnt[1:2])
+    ctx.push_deposit_compact(A, B, f_t, ctx.zeros(3), dt, na)
+    ctx.set_removed_counter(None)
+    ctx.set_clock_probe(None)
+    ctx.push_deposit(G.Particles.from_numpy(ptc), f_t, ctx.zeros(3), dt)       # no counter: nothing added
+    torch.cuda.synchronize()
+    assert cnt.cpu().tolist() == [n_gone, n_gone]
