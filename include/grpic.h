@@ -78,7 +78,9 @@ enum {
 };
 #define GRPIC_STATUS_FAR_MOVE 1u   /* a particle moved more than one cell in a step (still deposited exactly) */
 #define GRPIC_STATUS_NONFINITE 2u  /* a particle state became NaN/Inf (particle is flagged removed)           */
-#define GRPIC_STATUS_OFFGRID 4u    /* a deposit window left the guard region (contribution dropped)           */
+#define GRPIC_STATUS_OFFGRID 4u    /* a deposit window left the guard region (contribution dropped), or an active
+                                      particle was handed in outside [xi_in, xi_out) x [0, pi] (it is flagged
+                                      removed, its cell is clamped for the gather, nothing is deposited)      */
 #define GRPIC_STATUS_CAPACITY 8u   /* grpic_pair_production created more particles than the arrays hold       */
 
 /* Create a context: validates params, computes on the device the area elements of Eq.(8)
@@ -110,7 +112,11 @@ int grpic_set_workspace(grpic_ctx* ctx, void* dev_ptr, size_t bytes);
  * theta ghost rows receive the parts deposited beyond the domain).  `fields` must have
  * valid guard / ghost values (grpic_field_step and grpic_fill_guards maintain them).
  * `status` may be NULL.  The particle arrays must be 16-byte aligned (they are streamed
- * through shared memory with bulk TMA copies); otherwise GRPIC_ERR_ARG. */
+ * through shared memory with bulk TMA copies); otherwise GRPIC_ERR_ARG.  Particles that leave are
+ * only FLAGGED (bit 1) here; see grpic_set_removed_counter for the lazy-removal scheme and
+ * grpic_push_deposit_compact for compaction fused into the push.  On grids whose cells are no larger
+ * than 2^-8 in ln r and theta, at a time step with 2 dt <= 2^-8 r_in, r, sin(theta), cos(theta) are
+ * taken from the context's node tables plus a short in-cell series (a few ulp from exp / sincos). */
 int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                        grpic_current* flux, double dt, uint32_t* status, void* stream);
 
