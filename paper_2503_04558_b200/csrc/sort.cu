@@ -90,25 +90,59 @@ __device__ __forceinline__ uint32_t make_key(uint32_t cell, uint32_t flag, uint3
   return (flag & 2u) ? ncells : min(cell, ncells);
 }
 
-// per-tile digit histogram -> hist[digit*ntiles + tile]
+// per-tile digit histogram -> hist[digit*ntiles + tile].  Every thread takes 8 CONSECUTIVE keys (two
+// 16-byte loads), merges runs of equal digit among them (in the last pass, and in the first one of
+// an already cell-ordered array, all eight are usually equal) and adds each run once to its warp's
+// private histogram in shared memory; thread d then sums the eight warp histograms of digit d.
 template <bool FIRST>
 __global__ void __launch_bounds__(kThreads)
 radix_hist_kernel(const uint32_t* keys, const uint32_t* cell, const uint32_t* flag, int64_t n,
                   uint32_t ncells, int shift, uint32_t* hist, uint32_t ntiles) {
-  __shared__ uint32_t sh[kRadix];
-  sh[threadIdx.x] = 0;
-  __syncthreads();
-  const int64_t base = (int64_t)blockIdx.x * kTile;
+  __shared__ uint32_t sh[kThreads / 32][kRadix];
+  const int w = threadIdx.x >> 5;
 #pragma unroll
-  for (int m = 0; m < kTile / kThreads; ++m) {
-    const int64_t e = base + m * kThreads + threadIdx.x;
-    if (e < n) {
-      const uint32_t key = FIRST ? make_key(cell[e], flag[e], ncells) : keys[e];
-      atomicAdd(&sh[(key >> shift) & 0xFFu], 1u);
+  for (int q = 0; q < kThreads / 32; ++q) sh[q][threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t e0 = (int64_t)blockIdx.x * kTile + (int64_t)threadIdx.x * 8;
+  uint32_t k[8];
+  int cnt = 0;
+  // the caller's cell / flag arrays are only promised 4-byte alignment: vector loads if they have 16
+  const bool vec = !FIRST || ((((uintptr_t)cell | (uintptr_t)flag) & 15u) == 0);
+  if (e0 + 8 <= n && vec) {
+    cnt = 8;
+    if (FIRST) {
+      const uint4 c0 = *reinterpret_cast<const uint4*>(cell + e0), c1 = *reinterpret_cast<const uint4*>(cell + e0 + 4);
+      const uint4 f0 = *reinterpret_cast<const uint4*>(flag + e0), f1 = *reinterpret_cast<const uint4*>(flag + e0 + 4);
+      k[0] = make_key(c0.x, f0.x, ncells); k[1] = make_key(c0.y, f0.y, ncells);
+      k[2] = make_key(c0.z, f0.z, ncells); k[3] = make_key(c0.w, f0.w, ncells);
+      k[4] = make_key(c1.x, f1.x, ncells); k[5] = make_key(c1.y, f1.y, ncells);
+      k[6] = make_key(c1.z, f1.z, ncells); k[7] = make_key(c1.w, f1.w, ncells);
+    } else {
+      const uint4 a = *reinterpret_cast<const uint4*>(keys + e0), b = *reinterpret_cast<const uint4*>(keys + e0 + 4);
+      k[0] = a.x; k[1] = a.y; k[2] = a.z; k[3] = a.w; k[4] = b.x; k[5] = b.y; k[6] = b.z; k[7] = b.w;
+    }
+  } else {
+    for (int m = 0; m < 8; ++m)
+      if (e0 + m < n) { k[m] = FIRST ? make_key(cell[e0 + m], flag[e0 + m], ncells) : keys[e0 + m]; cnt = m + 1; }
+  }
+  uint32_t run_d = 0, run_n = 0;
+#pragma unroll
+  for (int m = 0; m < 8; ++m) {
+    if (m < cnt) {
+      const uint32_t d = (k[m] >> shift) & 0xFFu;
+      if (run_n && d == run_d) { ++run_n; }
+      else {
+        if (run_n) atomicAdd(&sh[w][run_d], run_n);
+        run_d = d; run_n = 1;
+      }
     }
   }
+  if (run_n) atomicAdd(&sh[w][run_d], run_n);
   __syncthreads();
-  hist[(size_t)threadIdx.x * ntiles + blockIdx.x] = sh[threadIdx.x];
+  uint32_t tot = 0;
+#pragma unroll
+  for (int q = 0; q < kThreads / 32; ++q) tot += sh[q][threadIdx.x];
+  hist[(size_t)threadIdx.x * ntiles + blockIdx.x] = tot;
 }
 
 // stable scatter of one tile: warp w owns keys [w*256, w*256+256) of the tile in 8 groups.
