@@ -143,11 +143,15 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
   // first iteration, 12 for the diagnostics mode) bulk copies with warp-uniform addresses.  (Round 1
   // let lanes 0..17 issue one copy each: ptxas serialises such divergent UBLKCP issue in an
   // ELECT / R2UR / BRA.U loop, ~160 of the 613 instructions per row, profiles/r02_final.md.) ----
+  // MODE 0 (predictor): the base of row jj-1 IS the iterate of row jj-1, which the previous iteration
+  // read: it is carried in registers (Fp) instead of being fetched again, and its six slots of the
+  // packet take the three J rows instead (no load is issued from inside the epilogue any more)
+  const bool jt = TMA && MODE == 0 && A.J[0] && A.J[1] && A.J[2];
   auto request = [&](int jj, int stage) {               // packet jj -> ring stage
     if (jj > jend) return;
     const bool epi = (jj - 1 >= jstart);                // epilogue operands of row jj-1 wanted
     if (elect_one()) {
-      const uint32_t nseg = epi ? (MODE != 2 ? 18u : 12u) : 6u;
+      const uint32_t nseg = epi ? (MODE == 1 ? 18u : MODE == 0 ? (jt ? 15u : 12u) : 12u) : 6u;
       const uint32_t bar32 = smem_u32(&bars[stage]);
       const uint32_t dst32 = smem_u32(ring) + (uint32_t)stage * (kSeg * 256u);
       mbar_expect_tx(&bars[stage], nseg * 256u);
@@ -158,9 +162,13 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
 #pragma unroll
       for (int c = 0; c < 6; ++c) tma_load_raw(dst32 + c * 256u, (uint64_t)A.in[c] + off0, bar32);
       if (epi) {
-        if (MODE != 2) {
+        if (MODE == 1) {
 #pragma unroll
           for (int c = 0; c < 6; ++c) tma_load_raw(dst32 + (6 + c) * 256u, (uint64_t)A.base[c] + off1, bar32);
+        }
+        if (MODE == 0 && jt) {
+#pragma unroll
+          for (int c = 0; c < 3; ++c) tma_load_raw(dst32 + (6 + c) * 256u, (uint64_t)A.J[c] + off1, bar32);
         }
         tma_load_raw(dst32 + 12 * 256u, (uint64_t)g.iADr + off1, bar32);
         tma_load_raw(dst32 + 13 * 256u, (uint64_t)g.iADth + off1, bar32);
@@ -191,6 +199,7 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
   double Hph_p = 0, Hph_im1_p = 0, Hr_p = 0, Hth_p = 0, Hth_im1_p = 0;
   double Eph_p = 0, Eph_ip1_p = 0, Er_p = 0, Eth_p = 0, Eth_ip1_p = 0;
   double Hph_pp = 0, Hr_pp = 0;
+  double Fp[6] = {0, 0, 0, 0, 0, 0};                    // MODE 0 with TMA: F^n of the previous row
 
   for (int jj = jstart - 1; jj <= jend; ++jj) {
     // ---- auxiliary fields of row jj ----
@@ -198,6 +207,7 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
     const int nit = jj - (jstart - 1);
     const int stg = nit % kStages;
     const double* rs = ring + (stg * kSeg) * 32 + lane;            // this iteration's ring stage
+    double Fin[6];
     {
       const size_t k = g.idx(ic, jj);
       if (!TMA && A.prefetch) {
@@ -223,6 +233,7 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
       const double Dr = TMA ? rs[0] : __ldg(A.in[0] + k), Dth = TMA ? rs[32] : __ldg(A.in[1] + k);
       const double Dph = TMA ? rs[64] : __ldg(A.in[2] + k), Br = TMA ? rs[96] : __ldg(A.in[3] + k);
       const double Bth = TMA ? rs[128] : __ldg(A.in[4] + k), Bph = TMA ? rs[160] : __ldg(A.in[5] + k);
+      Fin[0] = Dr; Fin[1] = Dth; Fin[2] = Dph; Fin[3] = Br; Fin[4] = Bth; Fin[5] = Bph;
       const double sn = __ldg(g.sin_n + jj + g.j0), cn = __ldg(g.cos_n + jj + g.j0);
       const double sh = __ldg(g.sin_h + jj + g.j0), ch = __ldg(g.cos_h + jj + g.j0);
       const Coef knn = coef_at(g, r_n, sn, cn), khn = coef_at(g, r_h, sn, cn);
@@ -285,8 +296,8 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
         if (MODE == 2) {
           v = ok[c] ? C[c] : 0.0;
         } else if (MODE == 0) {
-          const double Fn = TMA ? rs[(6 + c) * 32] : __ldg(A.base[c] + k);
-          const double Jc = (c < 3 && A.J[c]) ? __ldg(A.J[c] + k) : 0.0;
+          const double Fn = TMA ? Fp[c] : __ldg(A.base[c] + k);
+          const double Jc = (c < 3 && A.J[c]) ? (jt ? rs[(6 + c) * 32] : __ldg(A.J[c] + k)) : 0.0;
           v = ok[c] ? fma(A.dt, C[c] - Jc, Fn) : 0.0;
           if (A.base_out[c] && rowok && (FAST || i <= hi[c]))
             A.base_out[c][k] = ok[c] ? fma(A.dt, A.a_impl * C[c] - Jc, Fn) : 0.0;
@@ -313,6 +324,10 @@ __device__ __forceinline__ void sweep_rows(const GridDev& g, const SweepArgs& A,
       request(jj + kStages, stg);
     }
     // ---- rotate rows ----
+    if (MODE == 0 && TMA) {
+#pragma unroll
+      for (int c = 0; c < 6; ++c) Fp[c] = Fin[c];
+    }
     Hph_pp = Hph_p; Hr_pp = Hr_p;
     Hph_p = Hph; Hph_im1_p = Hph_im1; Hr_p = Hr; Hth_p = Hth; Hth_im1_p = Hth_im1;
     Eph_p = Eph; Eph_ip1_p = Eph_ip1; Er_p = Er; Eth_p = Eth; Eth_ip1_p = Eth_ip1;
@@ -495,6 +510,14 @@ int grpic_field_step(grpic_ctx* ctx, grpic_fields* fields, const grpic_current* 
   static int tma = -1;
   if (tma < 0) { const char* e = getenv("GRPIC_FS_TMA"); tma = e ? atoi(e) : 1; }
   A.tma = tma;
+  {
+    // bulk copies need 16-byte aligned row segments: element i = 0 is 32-byte aligned in arrays that
+    // start on a 32-byte boundary (grpic.h); a caller's view that does not takes the load path
+    uintptr_t bits = (uintptr_t)ws;
+    for (int c = 0; c < 6; ++c) bits |= (uintptr_t)F[c];
+    if (J) bits |= (uintptr_t)J->Fr | (uintptr_t)J->Fth | (uintptr_t)J->Fph;
+    if (bits & 15u) A.tma = 0;
+  }
   A.dt = dt;
   A.b_impl = ctx->p.beta_impl;
   A.a_impl = 1.0 - ctx->p.beta_impl;
