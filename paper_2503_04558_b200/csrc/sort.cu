@@ -48,24 +48,57 @@ __device__ __forceinline__ uint32_t block_excl_scan8(uint32_t v[8], uint32_t* sm
   }
   return smem[8];
 }
-__global__ void __launch_bounds__(kThreads) scan_tiles_kernel(uint32_t* data, size_t n, uint32_t* sums) {
-  __shared__ uint32_t sm[9];
+// eight consecutive words of one thread: two 16-byte accesses when the array is 16-byte aligned and
+// all eight are inside, else word by word (zeros beyond n)
+__device__ __forceinline__ void load8(const uint32_t* data, size_t base, size_t n, uint32_t v[8]) {
+  if (base + 8 <= n && (((uintptr_t)data) & 15u) == 0) {
+    const uint4 a = *reinterpret_cast<const uint4*>(data + base), b = *reinterpret_cast<const uint4*>(data + base + 4);
+    v[0] = a.x; v[1] = a.y; v[2] = a.z; v[3] = a.w; v[4] = b.x; v[5] = b.y; v[6] = b.z; v[7] = b.w;
+  } else {
+#pragma unroll
+    for (int m = 0; m < 8; ++m) v[m] = (base + m < n) ? data[base + m] : 0u;
+  }
+}
+__device__ __forceinline__ void store8(uint32_t* data, size_t base, size_t n, const uint32_t v[8]) {
+  if (base + 8 <= n && (((uintptr_t)data) & 15u) == 0) {
+    *reinterpret_cast<uint4*>(data + base) = make_uint4(v[0], v[1], v[2], v[3]);
+    *reinterpret_cast<uint4*>(data + base + 4) = make_uint4(v[4], v[5], v[6], v[7]);
+  } else {
+#pragma unroll
+    for (int m = 0; m < 8; ++m)
+      if (base + m < n) data[base + m] = v[m];
+  }
+}
+// sums[b] = sum of tile b (read only)
+__global__ void __launch_bounds__(kThreads) tile_sums_kernel(const uint32_t* data, size_t n, uint32_t* sums) {
+  __shared__ uint32_t sm[kThreads / 32];
   const size_t base = (size_t)blockIdx.x * kScanTile + (size_t)threadIdx.x * 8;
   uint32_t v[8];
+  load8(data, base, n, v);
+  uint32_t t = 0;
 #pragma unroll
-  for (int m = 0; m < 8; ++m) v[m] = (base + m < n) ? data[base + m] : 0u;
-  const uint32_t tot = block_excl_scan8(v, sm);
+  for (int m = 0; m < 8; ++m) t += v[m];
 #pragma unroll
-  for (int m = 0; m < 8; ++m)
-    if (base + m < n) data[base + m] = v[m];
-  if (threadIdx.x == 0 && sums) sums[blockIdx.x] = tot;
+  for (int d = 16; d > 0; d >>= 1) t += __shfl_xor_sync(0xffffffffu, t, d);
+  if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = t;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t tot = 0;
+    for (int q = 0; q < kThreads / 32; ++q) tot += sm[q];
+    sums[blockIdx.x] = tot;
+  }
 }
-__global__ void __launch_bounds__(kThreads) scan_add_kernel(uint32_t* data, size_t n, const uint32_t* sums) {
-  const uint32_t off = sums[blockIdx.x];
+// exclusive scan of every tile in place, plus the tile's offset offs[b] (nullable)
+__global__ void __launch_bounds__(kThreads) scan_tiles_kernel(uint32_t* data, size_t n, const uint32_t* offs) {
+  __shared__ uint32_t sm[9];
   const size_t base = (size_t)blockIdx.x * kScanTile + (size_t)threadIdx.x * 8;
+  const uint32_t off = offs ? offs[blockIdx.x] : 0u;
+  uint32_t v[8];
+  load8(data, base, n, v);
+  block_excl_scan8(v, sm);
 #pragma unroll
-  for (int m = 0; m < 8; ++m)
-    if (base + m < n) data[base + m] += off;
+  for (int m = 0; m < 8; ++m) v[m] += off;
+  store8(data, base, n, v);
 }
 }  // namespace
 // In-place exclusive scan of data[0..n); scratch must hold >= n/2048 + n/2048^2 + 8 words.
@@ -76,11 +109,13 @@ int grpic_exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream
     grpic_count_launches(1);
     return grpic_launch_ok();
   }
+  // reduce - scan the tile sums - scan the tiles with their offsets: the data is read twice and
+  // written once (the round-1 form scanned, then added: two reads, two writes, word by word)
   grpic_count_launches(2);
-  scan_tiles_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
+  tile_sums_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
   int rc = grpic_exclusive_scan(scratch, nb, scratch + nb, st);
   if (rc != GRPIC_OK) return rc;
-  scan_add_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
+  scan_tiles_kernel<<<(unsigned)nb, kThreads, 0, st>>>(data, n, scratch);
   return grpic_launch_ok();
 }
 namespace {
@@ -168,16 +203,26 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
   const int64_t tbase = (int64_t)blockIdx.x * kTile;
   const int64_t wbase = tbase + (int64_t)w * (kGroups * 32);
   uint32_t key[kGroups], idx[kGroups], dig[kGroups];
+  // all sixteen loads first (written as key = flag & 2 ? ncells : min(cell, ncells) inside the loop,
+  // the compiler loads the flag, branches on it and only then loads the cell: sixteen dependent
+  // round trips, 1.05 ms for the first pass against 0.57 for the second at 1e8 keys)
 #pragma unroll
   for (int q = 0; q < kGroups; ++q) {
     const int64_t e = wbase + q * 32 + lane;
-    if (e < n) {
-      key[q] = FIRST ? make_key(cell[e], flag[e], ncells) : keys_in[e];
-      idx[q] = FIRST ? (uint32_t)e : idx_in[e];
-      dig[q] = (key[q] >> shift) & 0xFFu;
-    } else {
-      key[q] = 0; idx[q] = 0; dig[q] = 0x100u;   // sentinel: never ranked or written
+    const int64_t es = e < n ? e : 0;
+    key[q] = FIRST ? cell[es] : keys_in[es];
+    idx[q] = FIRST ? flag[es] : idx_in[es];
+  }
+#pragma unroll
+  for (int q = 0; q < kGroups; ++q) {
+    const int64_t e = wbase + q * 32 + lane;
+    if (FIRST) {
+      const uint32_t c = min(key[q], ncells);
+      key[q] = (idx[q] & 2u) ? ncells : c;
+      idx[q] = (uint32_t)e;
     }
+    dig[q] = (key[q] >> shift) & 0xFFu;
+    if (e >= n) { key[q] = 0; idx[q] = 0; dig[q] = 0x100u; }   // sentinel: never ranked or written
   }
   // 1. per-warp digit counts
 #pragma unroll
@@ -245,16 +290,25 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
   }
 }
 
-__global__ void gather_particles_kernel(grpic_particles in, grpic_particles out, const uint32_t* perm,
-                                        uint32_t* perm_out) {
+// Payload move by the final permutation.  All nine loads are issued before the first store: the
+// arrays carry no no-alias promise, so written as nine copy statements the compiler keeps every
+// load behind the previous store (ten dependent memory round trips per thread; 2.88 ms at 1e8
+// particles against the time noted in profiles/r02_final.md for this form).
+__global__ void __launch_bounds__(256)
+gather_particles_kernel(grpic_particles in, grpic_particles out, const uint32_t* __restrict__ perm,
+                        uint32_t* __restrict__ perm_out) {
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= in.n) return;
   const uint32_t s = perm[k];
-  out.x1[k] = in.x1[s]; out.x2[k] = in.x2[s]; out.x3[k] = in.x3[s];
-  out.u1[k] = in.u1[s]; out.u2[k] = in.u2[s]; out.u3[k] = in.u3[s];
-  out.w[k] = in.w[s];
-  out.cell[k] = in.cell[s];
-  out.flag[k] = in.flag[s];
+  const double x1 = in.x1[s], x2 = in.x2[s], x3 = in.x3[s];
+  const double u1 = in.u1[s], u2 = in.u2[s], u3 = in.u3[s];
+  const double w = in.w[s];
+  const uint32_t cell = in.cell[s], flag = in.flag[s];
+  out.x1[k] = x1; out.x2[k] = x2; out.x3[k] = x3;
+  out.u1[k] = u1; out.u2[k] = u2; out.u3[k] = u3;
+  out.w[k] = w;
+  out.cell[k] = cell;
+  out.flag[k] = flag;
   if (perm_out) perm_out[k] = s;
 }
 
@@ -311,11 +365,15 @@ compact_scatter_kernel(grpic_particles in, grpic_particles out, const uint32_t* 
     const int64_t e = wbase + q * 32 + lane;
     if (ballots[q] & (1u << lane)) {
       const uint32_t d = off + __popc(ballots[q] & lt);
-      out.x1[d] = in.x1[e]; out.x2[d] = in.x2[e]; out.x3[d] = in.x3[e];
-      out.u1[d] = in.u1[e]; out.u2[d] = in.u2[e]; out.u3[d] = in.u3[e];
-      out.w[d] = in.w[e];
-      out.cell[d] = in.cell[e];
-      out.flag[d] = in.flag[e];
+      const double x1 = in.x1[e], x2 = in.x2[e], x3 = in.x3[e];      // loads before stores (see
+      const double u1 = in.u1[e], u2 = in.u2[e], u3 = in.u3[e];      // gather_particles_kernel)
+      const double w8 = in.w[e];
+      const uint32_t cell = in.cell[e], flag = in.flag[e];
+      out.x1[d] = x1; out.x2[d] = x2; out.x3[d] = x3;
+      out.u1[d] = u1; out.u2[d] = u2; out.u3[d] = u3;
+      out.w[d] = w8;
+      out.cell[d] = cell;
+      out.flag[d] = flag;
     }
     off += __popc(ballots[q]);
   }
@@ -339,15 +397,29 @@ bool ptc_ok(const grpic_particles* p) {
 // ------------------------------------------------------------------ contention-free cell order
 // start[c] = first position of key c in the sorted key array (lower bound), c in [0, ncells + 1]:
 // start[ncells] = first removed particle, start[ncells + 1] = n.
-__global__ void cell_start_kernel(const uint32_t* keys, uint32_t n, uint32_t ncells, uint32_t* start) {
-  const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-  if (c > ncells + 1) return;
-  uint32_t lo = 0, hi = n;                         // first k with keys[k] >= c
-  while (lo < hi) {
-    const uint32_t mid = lo + ((hi - lo) >> 1);
-    if (keys[mid] < c) lo = mid + 1; else hi = mid;
+// One thread per four sorted keys: wherever the key steps up from a to b at position k, start[c] = k
+// for every c in (a, b]; position n closes the list with the sentinel ncells + 1.  (Streams the keys
+// once; the round-1 form was a binary search per cell: 27 dependent loads, 132 us at 1e8 keys.)
+__global__ void __launch_bounds__(256)
+cell_start_kernel(const uint32_t* __restrict__ keys, uint32_t n, uint32_t ncells, uint32_t* __restrict__ start) {
+  const uint64_t k0 = 4ull * ((uint64_t)blockIdx.x * blockDim.x + threadIdx.x);
+  if (k0 > n) return;
+  uint32_t kv[4];
+  if (k0 + 4 <= n && (((uintptr_t)keys) & 15u) == 0) {
+    const uint4 a = *reinterpret_cast<const uint4*>(keys + k0);
+    kv[0] = a.x; kv[1] = a.y; kv[2] = a.z; kv[3] = a.w;
+  } else {
+#pragma unroll
+    for (int m = 0; m < 4; ++m) kv[m] = (k0 + m < n) ? keys[k0 + m] : ncells + 1u;
   }
-  start[c] = lo;
+  uint32_t lo = k0 == 0 ? 0u : keys[k0 - 1] + 1u;      // first cell whose start is not yet known
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    if (k0 + m <= n) {
+      for (uint32_t c = lo; c <= kv[m]; ++c) start[c] = (uint32_t)(k0 + m);
+      lo = kv[m] + 1u;
+    }
+  }
 }
 // Inside every block of B consecutive cells the particles are re-ordered rank-major: first the
 // first particle of each cell, then the second of each, ...  (rank = position among the particles
@@ -357,8 +429,8 @@ __global__ void cell_start_kernel(const uint32_t* keys, uint32_t n, uint32_t nce
 // 5.55 ms for this one at 1e8 particles, profiles/r02f).  One warp owns 32 consecutive cells
 // (32 / B blocks), lane = cell; perm2[dest] = perm[start[cell] + rank].
 __global__ void __launch_bounds__(256)
-interleave_perm_kernel(const uint32_t* perm, const uint32_t* start, uint32_t n, uint32_t ncells, uint32_t B,
-                       uint32_t* perm2) {
+interleave_perm_kernel(const uint32_t* __restrict__ perm, const uint32_t* __restrict__ start, uint32_t n,
+                       uint32_t ncells, uint32_t B, uint32_t* __restrict__ perm2) {
   const uint32_t lane = threadIdx.x & 31u;
   const uint32_t cell = (blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5)) * 32u + lane;
   const uint32_t s = cell < ncells ? start[cell] : 0u;
@@ -370,11 +442,17 @@ interleave_perm_kernel(const uint32_t* perm, const uint32_t* start, uint32_t n, 
 #pragma unroll
   for (int d = 16; d > 0; d >>= 1) maxc = max(maxc, __shfl_xor_sync(0xffffffffu, maxc, d));
   const uint32_t lt = (1u << lane) - 1u;
-  for (uint32_t r = 0; r < maxc; ++r) {
-    const bool act = cnt > r;
-    const uint32_t gb = __ballot_sync(0xffffffffu, act) & gmask;
-    if (act) perm2[dest + __popc(gb & lt)] = perm[s + r];
-    dest += __popc(gb);
+  for (uint32_t r0 = 0; r0 < maxc; r0 += 4) {               // four ranks per trip: four loads in flight
+    uint32_t v[4];
+#pragma unroll
+    for (uint32_t m = 0; m < 4; ++m) v[m] = (cnt > r0 + m) ? perm[s + r0 + m] : 0u;
+#pragma unroll
+    for (uint32_t m = 0; m < 4; ++m) {
+      const bool act = cnt > r0 + m;
+      const uint32_t gb = __ballot_sync(0xffffffffu, act) & gmask;
+      if (act) perm2[dest + __popc(gb & lt)] = v[m];
+      dest += __popc(gb);
+    }
   }
   // removed particles keep their stable order at the tail
   const uint32_t t0 = start[ncells];
@@ -431,7 +509,7 @@ int sort_impl(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, u
   if (interleave) {
     // (moving the payload inside the rank loop instead of writing perm2 first was measured: 24.7 ms
     // against 6.7 ms -- the loop is latency-bound, the separate gather runs at 4.6 TB/s)
-    cell_start_kernel<<<(ncells + 2 + 255) / 256, 256, 0, st>>>(kin, (uint32_t)n, ncells, start);
+    cell_start_kernel<<<(unsigned)(((uint64_t)n / 4 + 1 + 255) / 256), 256, 0, st>>>(kin, (uint32_t)n, ncells, start);
     interleave_perm_kernel<<<(ncells + 255) / 256, 256, 0, st>>>(iin, start, (uint32_t)n, ncells, (uint32_t)interleave, iout);
     uint32_t* t = iin; iin = iout; iout = t;
     grpic_count_launches(2);
