@@ -733,6 +733,32 @@ def test_sort_interleaved_bit_exact(G, O, n, B):
             assert np.array_equal(got[k], ptc[k][pref]), k
 
 
+@pytest.mark.parametrize("n,frac", [(4096, 0.0), (4096, 1.0), (5, 1.0), (4100, 0.5)])
+def test_sort_interleaved_degenerate_removal(G, O, n, frac):
+    """No particle removed, every particle removed, half of them: both sorts against the oracle
+    (the list of cell starts is closed by the position of the first removed particle and by n)."""
+    p = inputs.grid_params(32, 32, 0.9)
+    ctx = G.Context(p, n)
+    rng = np.random.default_rng(n)
+    ptc = inputs.make_particles(p, n, 13, "logical", ("loguniform", 0.1, 10.0))
+    ptc["flag"] = (ptc["flag"] | (2 * (rng.uniform(size=n) < frac))).astype(np.uint32)
+    src = G.Particles.from_numpy(ptc)
+    for B in (0, 8):
+        dst = G.Particles(n)
+        perm = torch.zeros(n, dtype=torch.int32, device="cuda")
+        if B:
+            ctx.sort_interleaved(src, dst, B, perm)
+            pref = O.sort_interleaved(ptc["cell"], ptc["flag"], p["nr"] * p["nth"], B)
+        else:
+            ctx.sort(src, dst, perm)
+            pref = O.sort(ptc["cell"], ptc["flag"])
+        torch.cuda.synchronize()
+        assert np.array_equal(perm.cpu().numpy().view(np.uint32), pref)
+        got = dst.to_numpy()
+        for k in ptc:
+            assert np.array_equal(got[k], ptc[k][pref]), k
+
+
 def test_config1_ten_coupled_steps(G, O):
     """BASELINE.json config 1 at full size: 128x128, 1e5 particles, 10 x (push+deposit,
     finalize, field step N=7)."""
@@ -979,6 +1005,33 @@ def test_field_step_full_size_parity(G, O, N):
             got = ctx.to_host(f_t[c])
             assert np.all(np.isfinite(got))
             assert grid_err(fo[c], got) <= 1e-11, (N, s, c, grid_err(fo[c], got))
+
+
+def test_field_step_arrays_off_the_16_byte_grid(G):
+    """Field and current arrays that start 8 bytes off a 16-byte boundary (a caller's view) cannot be
+    fetched by bulk copies: grpic_field_step takes its load path for them and gives bit-identical
+    results to the aligned call."""
+    cfg = inputs.config(4, nr=256, nth=192)
+    p, dt = cfg["params"], cfg["dt"]
+    ctx = G.Context(p, 16)
+    def shifted(t):
+        buf = torch.zeros(t.numel() + 1, dtype=torch.float64, device="cuda")
+        v = buf[1:].view(t.shape)
+        v.copy_(t)
+        assert v.data_ptr() % 16 == 8
+        return v
+    f_a = [ctx.to_device(x) for x in cfg["fields"]]
+    J_a = [ctx.to_device(x) for x in cfg["J"]]
+    bg = [ctx.to_device(x) for x in cfg["bg"]]
+    ctx.fill_guards(f_a)
+    f_b = [shifted(t) for t in f_a]
+    J_b = [shifted(t) for t in J_a]
+    for _ in range(2):
+        ctx.field_step(f_a, J_a, dt, bg)
+        ctx.field_step(f_b, J_b, dt, bg)
+    torch.cuda.synchronize()
+    for c in range(6):
+        assert torch.equal(f_a[c], f_b[c]), c
 
 
 def test_config3_full_size_interleaved_lazy_path(G, O):
