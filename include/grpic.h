@@ -74,7 +74,8 @@ enum {
   GRPIC_ERR_ARG = -1,       /* null pointer / out-of-range parameter                 */
   GRPIC_ERR_CUDA = -2,      /* CUDA runtime error (no device, launch failure, ...)   */
   GRPIC_ERR_WORKSPACE = -3, /* workspace missing or too small for this call          */
-  GRPIC_ERR_ALLOC = -4      /* could not allocate the context's own tables           */
+  GRPIC_ERR_ALLOC = -4,     /* could not allocate the context's own tables           */
+  GRPIC_ERR_TOO_LARGE = -5  /* size beyond the fixed capacity of a *_static entry point */
 };
 #define GRPIC_STATUS_FAR_MOVE 1u   /* a particle moved more than one cell in a step (still deposited exactly) */
 #define GRPIC_STATUS_NONFINITE 2u  /* a particle state became NaN/Inf (particle is flagged removed)           */
@@ -249,6 +250,22 @@ int grpic_sort_interleaved(grpic_ctx* ctx, const grpic_particles* in, grpic_part
 /* Order-preserving removal of flagged particles: survivors are copied to `out` (must not
  * alias `in`) in order; their count is written to the DEVICE word n_alive. */
 int grpic_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, int64_t* n_alive, void* stream);
+
+/* grpic_compact for callers that cannot allocate (CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same result bit for bit, but NO workspace -- neither
+ * grpic_set_workspace nor any cudaMalloc / cudaFree / allocating library call.  The scratch (per-tile
+ * survivor counts and their scan) lives in a file-scope `static __device__` array of the library,
+ * 160 KiB that every GPU that loads the library holds until exit, sized for at most
+ * GRPIC_COMPACT_STATIC_MAX_PARTICLES particles: in->n beyond that returns GRPIC_ERR_TOO_LARGE and
+ * launches nothing.  ALL calls on one device share that array: calls that overlap on the GPU (two
+ * streams, two contexts, two host threads) race and give wrong results -- serialise them.  The array
+ * keeps the last call's contents; nothing in it has to start at zero (every word a call reads was
+ * written by that call first).  The first call on each device resolves the array's device address
+ * (cudaGetSymbolAddress, no allocation): make that first call outside stream capture, with the device
+ * of the arrays current. */
+#define GRPIC_COMPACT_STATIC_MAX_PARTICLES (1 << 26)
+int grpic_compact_static(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, int64_t* n_alive,
+                         void* stream);
 
 /* Charge density on vertices, rho_ij = sum q w S_ij(x) / dV_ij (theta ghosts folded);
  * divide = 0 returns rho*dV.  Overwrites `rho`. */

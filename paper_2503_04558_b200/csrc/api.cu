@@ -325,6 +325,7 @@ const char* grpic_strerror(int code) {
     case GRPIC_ERR_CUDA: return "CUDA runtime error (no device or launch failure)";
     case GRPIC_ERR_WORKSPACE: return "workspace missing or too small";
     case GRPIC_ERR_ALLOC: return "allocation of context tables failed";
+    case GRPIC_ERR_TOO_LARGE: return "size beyond the fixed capacity of a *_static entry point";
     default: return "unknown grpic error";
   }
 }

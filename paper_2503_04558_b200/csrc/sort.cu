@@ -4,7 +4,16 @@
 // PAPER.md:138,:364.
 #include <stdlib.h>
 
+#include <mutex>
+
 #include "grpic_internal.cuh"
+
+// Scratch of grpic_compact_static: per-tile alive counts + the words of their scan, for at most
+// GRPIC_COMPACT_STATIC_MAX_PARTICLES particles (2^26 -> 32768 tiles of 2048 + 16 + 4096 words; 160 KiB
+// that every GPU that loads the library holds until exit).  In HOST code this name is a stand-in, not
+// a device address: static_scratch() below resolves it with cudaGetSymbolAddress once per device.
+constexpr size_t kStaticScratchWords = 40960;
+static __device__ __align__(256) uint32_t g_compact_static_scratch[kStaticScratchWords];
 
 namespace {
 
@@ -530,6 +539,58 @@ int grpic_sort_interleaved(grpic_ctx* ctx, const grpic_particles* in, grpic_part
                            int32_t block_cells, void* stream) {
   if (block_cells < 1 || block_cells > 32 || (block_cells & (block_cells - 1))) return GRPIC_ERR_ARG;
   return sort_impl(ctx, in, out, perm, block_cells, (cudaStream_t)stream);
+}
+
+// Device address of g_compact_static_scratch on the CURRENT device, resolved once per device (no
+// allocation: the array is part of the loaded module) and cached.
+static int static_scratch(uint32_t** out) {
+  constexpr int kMaxDevices = 64;
+  static uint32_t* cache[kMaxDevices] = {};
+  static std::mutex mu;
+  int dev = -1;
+  GRPIC_CUDA_OK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return GRPIC_ERR_CUDA;
+  std::lock_guard<std::mutex> lock(mu);
+  if (!cache[dev]) {
+    uint32_t* ptr = nullptr;
+    GRPIC_CUDA_OK(cudaGetSymbolAddress((void**)&ptr, g_compact_static_scratch));
+    if (!ptr) return GRPIC_ERR_CUDA;
+    cache[dev] = ptr;
+  }
+  *out = cache[dev];
+  return GRPIC_OK;
+}
+
+int grpic_compact_static(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, int64_t* n_alive,
+                         void* stream) {
+  if (!ctx || !ptc_ok(in) || !out || !n_alive) return GRPIC_ERR_ARG;
+  const int64_t n = in->n;
+  if (n > (int64_t)GRPIC_COMPACT_STATIC_MAX_PARTICLES) return GRPIC_ERR_TOO_LARGE;
+  out->n = n;
+  cudaStream_t st = (cudaStream_t)stream;
+  if (n == 0) {
+    GRPIC_CUDA_OK(cudaMemsetAsync(n_alive, 0, sizeof(int64_t), st));
+    return GRPIC_OK;
+  }
+  if (!ptc_ok(out) || out->x1 == in->x1) return GRPIC_ERR_ARG;
+  const uint32_t ntiles = (uint32_t)((n + kTile - 1) / kTile);
+  static_assert((GRPIC_COMPACT_STATIC_MAX_PARTICLES + kTile - 1) / kTile +
+                        (GRPIC_COMPACT_STATIC_MAX_PARTICLES + kTile - 1) / kTile / kScanTile + 4096 <=
+                    kStaticScratchWords,
+                "static scratch too small for GRPIC_COMPACT_STATIC_MAX_PARTICLES");
+  uint32_t* counts = nullptr;
+  int rc = static_scratch(&counts);
+  if (rc != GRPIC_OK) return rc;
+  // nothing in the scratch has to start at zero: alive_count writes counts[0, ntiles), the scan writes
+  // every tile sum before it reads it -- the previous call's contents are never read
+  uint32_t* scratch = counts + ntiles;
+  alive_count_kernel<<<ntiles, kThreads, 0, st>>>(in->flag, n, counts);
+  rc = grpic_exclusive_scan(counts, ntiles, scratch, st);
+  if (rc != GRPIC_OK) return rc;
+  compact_scatter_kernel<<<ntiles, kThreads, 0, st>>>(*in, *out, counts, ntiles, n_alive);
+  mark_tail_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(*out, n, n_alive);
+  grpic_count_launches(3);
+  return grpic_launch_ok();
 }
 
 int grpic_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out, int64_t* n_alive, void* stream) {

@@ -49,7 +49,7 @@ EXPORTS = ["grpic_create", "grpic_destroy", "grpic_grid_layout", "grpic_get_area
            "grpic_workspace_bytes", "grpic_set_workspace", "grpic_set_removed_counter", "grpic_set_flux_exchange", "grpic_push_deposit",
            "grpic_push_deposit_compact", "grpic_step_host", "grpic_pair_production", "grpic_push_deposit_spline3", "grpic_push_deposit_variant",
            "grpic_finalize_current", "grpic_field_step", "grpic_fill_guards",
-           "grpic_circulation", "grpic_ks_to_bl", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_deposit_rho",
+           "grpic_circulation", "grpic_ks_to_bl", "grpic_sort", "grpic_sort_interleaved", "grpic_compact", "grpic_compact_static", "grpic_deposit_rho",
            "grpic_measure_fp64_peak", "grpic_measure_fp64_peak_clocked", "grpic_set_clock_probe", "grpic_kernel_launches", "grpic_strerror"]
 
 _lib = None
@@ -349,6 +349,16 @@ class Context:
         a, b = src.struct(), dst.struct()
         _check(load().grpic_compact(self.h, C.byref(a), C.byref(b),
                                     C.cast(C.c_void_p(n_alive.data_ptr()), C.POINTER(C.c_int64)), _stream()))
+        dst.n = src.n
+
+    COMPACT_STATIC_MAX_PARTICLES = 1 << 26
+
+    def compact_static(self, src, dst, n_alive):
+        """grpic_compact without a workspace or any allocation (scratch in a static device array of the
+        library; at most COMPACT_STATIC_MAX_PARTICLES particles; calls must not overlap on the GPU)."""
+        a, b = src.struct(), dst.struct()
+        _check(load().grpic_compact_static(self.h, C.byref(a), C.byref(b),
+                                           C.cast(C.c_void_p(n_alive.data_ptr()), C.POINTER(C.c_int64)), _stream()))
         dst.n = src.n
 
     def ks_to_bl(self, ptc):
