@@ -194,15 +194,19 @@ radix_hist_kernel(const uint32_t* keys, const uint32_t* cell, const uint32_t* fl
 // counts + stable rank of the key among the tile's keys of that digit), then written out in that
 // order: all keys of one digit go to consecutive global positions, so every warp store covers whole
 // runs instead of 32 scattered 4-byte elements (pass 1 at 1e8 keys: 1.08 -> see profiles/r02_final.md).
+// resident CTAs per SM asked of the compiler (register cap 64): measured steady-state sort at 1e8
+// particles 5.25 / 5.39 / 5.72 ms for 4 / 5 / 6 (5 and 6 spill)
+#ifndef GRPIC_SCATTER_MINB
+#define GRPIC_SCATTER_MINB 4
+#endif
 template <bool FIRST>
-__global__ void __launch_bounds__(kThreads)
+__global__ void __launch_bounds__(kThreads, GRPIC_SCATTER_MINB)
 radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint32_t* cell,
                      const uint32_t* flag, int64_t n, uint32_t ncells, int shift,
                      const uint32_t* hist_scanned, uint32_t ntiles, uint32_t* keys_out,
                      uint32_t* idx_out) {
   __shared__ uint32_t whist[kThreads / 32][kRadix];   // per-warp digit counts, then local starts
-  __shared__ uint32_t tstart[kRadix];                  // exclusive prefix of the tile's digit counts
-  __shared__ uint32_t gstart[kRadix];                  // global start of the tile's run of each digit
+  __shared__ uint32_t gdelta[kRadix];                  // global start of the tile's run of a digit - its start in the tile
   __shared__ uint32_t skey[kTile], sidx[kTile];
   __shared__ uint32_t wsum[kThreads / 32];
   const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -212,6 +216,8 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
   const int64_t tbase = (int64_t)blockIdx.x * kTile;
   const int64_t wbase = tbase + (int64_t)w * (kGroups * 32);
   uint32_t key[kGroups], idx[kGroups], dig[kGroups];
+  // global start of the tile's run of digit threadIdx.x: asked for now, used in step 2
+  const uint32_t gs = hist_scanned[(size_t)threadIdx.x * ntiles + blockIdx.x];
   // all sixteen loads first (written as key = flag & 2 ? ncells : min(cell, ncells) inside the loop,
   // the compiler loads the flag, branches on it and only then loads the cell: sixteen dependent
   // round trips, 1.05 ms for the first pass against 0.57 for the second at 1e8 keys)
@@ -233,12 +239,20 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
     dig[q] = (key[q] >> shift) & 0xFFu;
     if (e >= n) { key[q] = 0; idx[q] = 0; dig[q] = 0x100u; }   // sentinel: never ranked or written
   }
-  // 1. per-warp digit counts
+  // 1. per-warp digit counts and, in the same sweep, the rank of every key among the keys of its
+  //    digit in its warp (input order: group by group, lane by lane).  One MATCH per key -- the
+  //    slowest instruction of the kernel -- and one shared-memory update per distinct digit of a group
+  const uint32_t lt = (1u << lane) - 1u;
+  uint32_t rank_q[kGroups];
 #pragma unroll
   for (int q = 0; q < kGroups; ++q) {
     const uint32_t peers = __match_any_sync(0xffffffffu, dig[q]);
-    if (dig[q] < kRadix && lane == (__ffs(peers) - 1)) whist[w][dig[q]] += __popc(peers);
+    const bool valid = dig[q] < kRadix;
+    const uint32_t before = valid ? whist[w][dig[q]] : 0u;
     __syncwarp();
+    if (valid && lane == (__ffs(peers) - 1)) whist[w][dig[q]] = before + __popc(peers);
+    __syncwarp();
+    rank_q[q] = before + __popc(peers & lt);
   }
   __syncthreads();
   // 2. thread d: tile count of digit d, exclusive prefix over the digits (block scan), local start
@@ -258,8 +272,8 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
     uint32_t off = 0;
     for (int q = 0; q < w; ++q) off += wsum[q];
     uint32_t run = off + incl - tot;                 // exclusive prefix of digit threadIdx.x
-    tstart[threadIdx.x] = run;
-    gstart[threadIdx.x] = hist_scanned[(size_t)threadIdx.x * ntiles + blockIdx.x];
+    // element e of the sorted tile, of digit d, goes to global position e + gdelta[d]
+    gdelta[threadIdx.x] = gs - run;
 #pragma unroll
     for (int q = 0; q < kThreads / 32; ++q) {
       const uint32_t cnt = whist[q][threadIdx.x];
@@ -268,31 +282,24 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
     }
   }
   __syncthreads();
-  // 3. rank inside the warp, group by group (keeps the input order of equal digits): position in
-  //    the tile's sorted order
-  const uint32_t lt = (1u << lane) - 1u;
+  // 3. position in the tile's sorted order = start of the warp's run of the digit + rank in the warp
 #pragma unroll
   for (int q = 0; q < kGroups; ++q) {
-    const uint32_t peers = __match_any_sync(0xffffffffu, dig[q]);
-    uint32_t pos = 0;
-    if (dig[q] < kRadix) pos = whist[w][dig[q]] + __popc(peers & lt);
-    __syncwarp();
-    if (dig[q] < kRadix && lane == (__ffs(peers) - 1)) whist[w][dig[q]] += __popc(peers);
-    __syncwarp();
     if (dig[q] < kRadix) {
+      const uint32_t pos = whist[w][dig[q]] + rank_q[q];
       skey[pos] = key[q];
       sidx[pos] = idx[q];
     }
   }
   __syncthreads();
-  // 4. write the tile in sorted order: element e of the tile goes to gstart[d] + (e - tstart[d])
+  // 4. write the tile in sorted order
   const uint32_t cnt_tile = (uint32_t)((n - tbase) < (int64_t)kTile ? (n - tbase) : (int64_t)kTile);
 #pragma unroll
   for (int m = 0; m < kTile / kThreads; ++m) {
     const uint32_t e = m * kThreads + threadIdx.x;
     if (e < cnt_tile) {
       const uint32_t k = skey[e], d = (k >> shift) & 0xFFu;
-      const uint32_t pos = gstart[d] + (e - tstart[d]);
+      const uint32_t pos = e + gdelta[d];
       keys_out[pos] = k;
       idx_out[pos] = sidx[e];
     }
