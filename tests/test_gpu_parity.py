@@ -363,14 +363,16 @@ def test_far_moves_take_the_general_window(G, O):
         assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
 
 
-def test_spline3_push_deposit_parity(G, O):
+@pytest.mark.parametrize("nr,nth,n", [(48, 40, 20000), (320, 256, 300007)])
+def test_spline3_push_deposit_parity(G, O, nr, nth, n):
     """third-order (cubic B-spline) shape option: gather, push and deposit vs the
-    oracle run with the same option; includes axis crossers, leavers and photons."""
-    p = inputs.grid_params(48, 40, 0.99, ng=3)
+    oracle run with the same option; includes axis crossers, leavers and photons.  The second size
+    spans many CTAs and a ragged tail."""
+    p = inputs.grid_params(nr, nth, 0.99, ng=3)
     dt = inputs.courant_dt(p)
     fields = inputs.analytic_fields(p, "wald")
-    ptc = inputs.make_particles(p, 20000, 23, "crowded", ("loguniform", 0.1, 1e3))
-    ptc["flag"] = (ptc["flag"] | np.where(np.arange(20000) % 7 == 0, 4, 0)).astype(np.uint32)
+    ptc = inputs.make_particles(p, n, 23, "crowded", ("loguniform", 0.1, 1e3))
+    ptc["flag"] = (ptc["flag"] | np.where(np.arange(n) % 7 == 0, 4, 0)).astype(np.uint32)
     with O.shape_order(3):
         ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
     ref1, Fref1 = oracle_push_deposit(O, p, fields, ptc, dt)
@@ -517,15 +519,17 @@ def test_gpu_coupled_loop_preserves_gauss_law(G, O):
     assert np.max(np.abs((g1 - g0)[sel])) < 1e-11 * sc, np.max(np.abs((g1 - g0)[sel])) / sc
 
 
-@pytest.mark.parametrize("order,pusher", [(1, 0), (1, 1), (3, 1)])
-def test_push_deposit_variants_parity(G, O, order, pusher):
+@pytest.mark.parametrize("order,pusher,nr,nth,n", [(1, 0, 48, 40, 20000), (1, 1, 48, 40, 20000), (3, 1, 48, 40, 20000),
+                                                   (1, 1, 320, 256, 300007), (3, 1, 320, 256, 300007)])
+def test_push_deposit_variants_parity(G, O, order, pusher, nr, nth, n):
     """grpic_push_deposit_variant vs the oracle with the same options: shape order 1 / 3
      and pusher Boris / Vay in the FIDO frame.  (1, 0) must also
-    agree with the tuned default kernel's result through the oracle."""
-    p = inputs.grid_params(48, 40, 0.99, ng=3)
+    agree with the tuned default kernel's result through the oracle.  The larger size spans many
+    CTAs and a ragged tail."""
+    p = inputs.grid_params(nr, nth, 0.99, ng=3)
     dt = inputs.courant_dt(p)
     fields = inputs.analytic_fields(p, "wald")
-    ptc = inputs.make_particles(p, 20000, 41, "crowded", ("loguniform", 0.1, 1e3))
+    ptc = inputs.make_particles(p, n, 41, "crowded", ("loguniform", 0.1, 1e3))
     with O.shape_order(order), O.pusher(pusher):
         ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
     ctx = G.Context(p, len(ptc["x1"]))
