@@ -151,6 +151,9 @@ def parse(argv=None):
                     help="cell sort order: rank-interleaved inside blocks of --sort-block cells "
                          "(grpic_sort_interleaved, contention-free deposit) or the plain stable order (grpic_sort)")
     ap.add_argument("--sort-block", type=int, default=8)
+    ap.add_argument("--variant", default="cic-boris", choices=["cic-boris", "cic-vay", "spline3-boris", "spline3-vay"],
+                    help="particle shape and momentum update (SURVEY.md 8(f) next-2 / next-3): the default is the "
+                         "tuned first-order / generalised-Boris kernel; the others go through grpic_push_deposit_variant")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -219,8 +222,9 @@ def workload(args, rank):
     k = args.config
     n = args.particles or None
     g = args.grid or None
+    ng = 3 if args.variant.startswith("spline3") else 2      # the cubic spline's support needs three guard nodes
     if rank > 0:  # a different seed per rank: patch the seed through make_particles
-        cfg = inputs.config(k, nr=g, nth=g, n=16)   # cheap: fields + params only
+        cfg = inputs.config(k, nr=g, nth=g, n=16, ng=ng)   # cheap: fields + params only
         recipe = {1: ("logical", ("loguniform", 0.1, 10.0), False, 100_000, 0),
                   2: ("r2", ("mj_tail", 1.0, 0.1, 10.0, 1e4), True, 20_000_000, 1),
                   3: ("crowded", ("loguniform", 0.1, 1e5), False, 100_000_000, 2),
@@ -228,7 +232,7 @@ def workload(args, rank):
         cfg["particles"] = inputs.make_particles(cfg["params"], n or recipe[3], rank_seed(k, rank),
                                                  recipe[0], recipe[1], pairs=recipe[2])
     else:
-        cfg = inputs.config(k, nr=g, nth=g, n=n)
+        cfg = inputs.config(k, nr=g, nth=g, n=n, ng=ng)
     return cfg
 
 
@@ -311,6 +315,10 @@ def run_ours(args):
     policy = "separate" if args.separate_compact else args.compaction
     if not compact:
         policy = "none"
+    variant = args.variant != "cic-boris"       # the method variants: general kernel, in place, flags only
+    v_order, v_pusher = (3 if args.variant.startswith("spline3") else 1), (1 if args.variant.endswith("vay") else 0)
+    if variant and policy in ("fused", "separate"):
+        policy = "sort"
     fused = policy == "fused"
     lazy = policy == "sort"
 
@@ -351,6 +359,8 @@ def run_ours(args):
         if fused:       # removal fused into the push: survivors of `cur` are pushed into `alt`
             ctx.push_deposit_compact(cur, alt, fields, flux, dt, n_alive[s:s + 1])
             cur, alt = alt, cur
+        elif variant:
+            ctx.push_deposit_variant(cur, fields, flux, dt, v_order, v_pusher)
         else:
             if lazy:
                 ctx.set_removed_counter(removed[s:s + 1])
@@ -379,6 +389,7 @@ def run_ours(args):
     barrier()
     setup_s = time.time() - t_setup
 
+    live0 = int((state[0].t["flag"] & 2 == 0).sum().item()) if variant else 0
     launches0 = ctx.kernel_launches()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
@@ -394,7 +405,10 @@ def run_ours(args):
     clocks = ClockSampler.summarise(sampler.window(tw0, tw1)) if sampler else None
 
     # particles actually pushed per timed step (alive at the start of the step)
-    if lazy:
+    if variant:        # the general kernel keeps no removal counter: live particles before / after, in between linear
+        live1 = int((state[0].t["flag"] & 2 == 0).sum().item())
+        pushed = [int(round(live0 + (live1 - live0) * q / K)) for q in range(K)]
+    elif lazy:
         ctx.set_removed_counter(None)
         gone = np.concatenate([[0], np.cumsum(removed.cpu().numpy())])
         pushed = [int(n - gone[s]) for s in range(W, W + K)]
@@ -454,7 +468,7 @@ def run_ours(args):
     rc = roofline_constants()
     fp64_pp = float(rc["fp64_instr_per_particle"])
     # the constants belong to one instantiation (K = 3 correctors, first-order shape, fine-grid TAB path)
-    applies = p["geo_iters"] == 3 and policy != "separate" and \
+    applies = not variant and p["geo_iters"] == 3 and policy != "separate" and \
         (("1, 3" in rc["kernel"] or "true, (int)3" in rc["kernel"]) == fused or "kernel" not in rc)
     fp64_ach = fp64_pp * per_launch / (pd_ms * 1e-3)
     hbm_ach = HBM_BYTES_PER_PARTICLE * per_launch / (pd_ms * 1e-3) / 1e9
@@ -552,6 +566,10 @@ def run_ours(args):
                                       "fused": "fused into every push (grpic_push_deposit_compact)",
                                       "separate": "separate pass every step (grpic_compact)",
                                       "none": "none"}[policy],
+                       "variant": {"cic-boris": "first-order shape, generalised Boris (tuned kernel)",
+                                   "cic-vay": "first-order shape, Vay pusher (grpic_push_deposit_variant)",
+                                   "spline3-boris": "cubic B-spline shape, generalised Boris (grpic_push_deposit_variant)",
+                                   "spline3-vay": "cubic B-spline shape, Vay pusher (grpic_push_deposit_variant)"}[args.variant],
                        "filter_passes": filt,
                        "field_step": True, "field_iters": p["field_iters"], "geo_iters": p["geo_iters"],
                        "macro_weight": BENCH_WEIGHT,

@@ -135,12 +135,15 @@ int grpic_set_removed_counter(grpic_ctx* ctx, unsigned long long* device_counter
  * the spline's support on each component's own lattice, prefix-sum deposit (Eq.21-23) over the
  * window the spline covers during the move.  In place, fluxes accumulated (+=) as in
  * grpic_push_deposit.  The context must have been created with ng >= 3 guard nodes
- * (GRPIC_ERR_ARG otherwise).  Parity-level implementation, not tuned. */
+ * (GRPIC_ERR_ARG otherwise).  General kernel (one thread per particle, 96 loads and up to 96 REDs per
+ * particle): about 4.5 x the time of the first-order step (profiles/r02_late_experiments.md). */
 int grpic_push_deposit_spline3(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields,
                                grpic_current* flux, double dt, uint32_t* status, void* stream);
 
 /* The particle step with the paper's method variants selected by argument (same in-place
- * semantics as grpic_push_deposit; general, untuned kernel):
+ * semantics as grpic_push_deposit).  (1, 1) runs the tuned kernel of grpic_push_deposit with the Vay
+ * update in place of Boris when the particle arrays are 16-byte aligned; everything else the general
+ * kernel:
  *   shape_order = 1 (cloud-in-cell) or 3 (cubic B-spline, needs ng >= 3);
  *   pusher = 0: generalised Boris (Eq.16-19); 1: Vay update in the FIDO frame (Vay
  *   2008) with the triad e_(1) = sqrt(gamma^rr)(d_r - gamma_rphi/gamma_phiphi d_phi),

@@ -308,18 +308,19 @@ def make_particles(p, n, seed, position="logical", momentum=("loguniform", 0.1, 
 
 
 # --------------------------------------------------------------------------- configs
-def config(k, scale=1.0, nr=None, nth=None, n=None):
+def config(k, scale=1.0, nr=None, nth=None, n=None, ng=2):
     """The five BASELINE.json configs (k = 1..5); `nr`, `nth`, `n` override the size for
-    reduced-size parity tests (the recipe is otherwise unchanged).
+    reduced-size parity tests (the recipe is otherwise unchanged); `ng` = guard nodes (3 for the
+    cubic-spline shape).
     Returns dict(params, dt, fields, particles, J, bg, meta)."""
     out = dict(J=None, bg=None, particles=None)
     if k == 1:
-        p = grid_params(nr or 128, nth or 128, 0.99)
+        p = grid_params(nr or 128, nth or 128, 0.99, ng=ng)
         out.update(params=p, dt=courant_dt(p), fields=split_monopole_fields(p),
                    particles=make_particles(p, n or 100_000, 0, "logical", ("loguniform", 0.1, 10.0)),
                    meta=dict(steps=10, sort_every=0, filter_passes=0, field=True))
     elif k == 2:
-        p = grid_params(nr or 1024, nth or 1024, 0.99)
+        p = grid_params(nr or 1024, nth or 1024, 0.99, ng=ng)
         rng = np.random.Generator(np.random.PCG64(1001))
         out.update(params=p, dt=courant_dt(p),
                    fields=fill_guards(p, perturb(analytic_fields(p, "wald"), 1e-3, rng)),
@@ -327,7 +328,7 @@ def config(k, scale=1.0, nr=None, nth=None, n=None):
                                             ("mj_tail", 1.0, 0.1, 10.0, 1e4), pairs=True),
                    meta=dict(steps=100, sort_every=20, filter_passes=0, field=False))
     elif k == 3:
-        p = grid_params(nr or 2048, nth or 2048, 0.99)
+        p = grid_params(nr or 2048, nth or 2048, 0.99, ng=ng)
         rng = np.random.Generator(np.random.PCG64(1002))
         out.update(params=p, dt=courant_dt(p),
                    fields=fill_guards(p, perturb(analytic_fields(p, "wald"), 1e-3, rng)),
@@ -335,7 +336,7 @@ def config(k, scale=1.0, nr=None, nth=None, n=None):
                                             ("loguniform", 0.1, 1e5)),
                    meta=dict(steps=50, sort_every=0, compact_every=1, filter_passes=0, field=False))
     elif k == 4:
-        p = grid_params(nr or 4096, nth or 4096, 0.9)
+        p = grid_params(nr or 4096, nth or 4096, 0.9, ng=ng)
         p["damp_cells"] = p["nr"] // 10
         p["damp_coef"] = 1.0
         rng = np.random.Generator(np.random.PCG64(3))
@@ -346,7 +347,7 @@ def config(k, scale=1.0, nr=None, nth=None, n=None):
                    J=random_current(p, rng),
                    meta=dict(steps=1000, sort_every=0, filter_passes=0, field=True))
     elif k == 5:
-        p = grid_params(nr or 2048, nth or 2048, 0.99)
+        p = grid_params(nr or 2048, nth or 2048, 0.99, ng=ng)
         out.update(params=p, dt=courant_dt(p), fields=analytic_fields(p, "monopole"),
                    particles=make_particles(p, n or 200_000_000, 4, "r2", ("mj", 0.1)),
                    meta=dict(steps=200, sort_every=10, filter_passes=3, field=True))

@@ -65,5 +65,9 @@ __device__ __forceinline__ double ks_sqrtg(double a2, double M, double r, double
 void grpic_count_launches(int n);
 // in-place exclusive scan of data[0..n) (sort.cu); scratch >= n/2048 + n/2048^2 + 8 words
 int grpic_exclusive_scan(uint32_t* data, size_t n, uint32_t* scratch, cudaStream_t st);
+// first-order shape + Vay pusher through the tuned kernel (push_deposit.cu); GRPIC_ERR_ARG if the arrays
+// do not allow its bulk-TMA tiles
+int grpic_push_deposit_cic_vay(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields, grpic_current* flux,
+                               double dt, uint32_t* status, cudaStream_t st);
 // frees the staging state of grpic_step_host (host_step.cu)
 void grpic_host_step_release(grpic_ctx* ctx);

@@ -178,7 +178,7 @@ constexpr uint32_t kTileBytes = 7u * kWTile * 8u + kWTile * 4u;
 // registers per thread for MINB resident 64-thread CTAs: 8 -> 128, 9 -> 112, 10 -> 96 (ptxas left to
 // itself picks 96 for MINB = 9)
 constexpr int pd_max_regs(int minb) { return minb <= 8 ? 128 : (minb == 9 ? 112 : 96); }
-template <int MINB, bool COMPACT, int KT, bool TAB>
+template <int MINB, bool COMPACT, int KT, bool TAB, bool VAY = false>
 __global__ void __launch_bounds__(kBlock) __maxnreg__(pd_max_regs(MINB))
 push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
                     const __grid_constant__ grpic_particles dst, const uint32_t* __restrict__ offsets,
@@ -362,7 +362,8 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     // ---- Boris (full dt) at x^n ----
     double ur = T.u1[sl], ut = T.u2[sl], up = T.u3[sl];
 #ifndef GRPIC_ABL_NO_BORIS
-    boris(g, p0, alpha0, sgn, dt, D, B, ur, ut, up);
+    if (VAY) vay(g, p0, alpha0, sgn, dt, D, B, ur, ut, up);      // PAPER.md:204, grpic_push_deposit_variant
+    else boris(g, p0, alpha0, sgn, dt, D, B, ur, ut, up);
 #else
     ur += 1e-300 * (D[0] + D[1] + D[2] + B[0] + B[1] + B[2]);     // keeps the gather alive
 #endif
@@ -497,20 +498,20 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   }
 }
 
-template <int MINB, bool COMPACT, int KT, bool TAB>
+template <int MINB, bool COMPACT, int KT, bool TAB, bool VAY = false>
 int launch_push_deposit(const grpic_ctx* ctx, const grpic_particles& ptc, const grpic_particles& dst,
                         const uint32_t* offsets, const grpic_fields& f,
                         const grpic_current& J, double dt, uint32_t* status, cudaStream_t st) {
   static int per_sm = 0;   // resident CTAs per SM of this instantiation
   if (per_sm == 0) {
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, COMPACT, KT, TAB>,
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, push_deposit_kernel<MINB, COMPACT, KT, TAB, VAY>,
                                                       kBlock, 0) != cudaSuccess || per_sm < 1)
       per_sm = 1;
   }
   const int64_t nblocks = (ptc.n + kWarps * kWTile - 1) / (kWarps * kWTile);
   const int64_t resident = (int64_t)ctx->sm_count * per_sm;
   const unsigned grid = (unsigned)(nblocks < resident ? nblocks : resident);
-  push_deposit_kernel<MINB, COMPACT, KT, TAB><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, f, J, kPolyTabHost, dt,
+  push_deposit_kernel<MINB, COMPACT, KT, TAB, VAY><<<grid, kBlock, 0, st>>>(ctx->g, ptc, dst, offsets, f, J, kPolyTabHost, dt,
                                                                   ctx->p.geo_iters, status, ctx->removed_counter,
                                                                   ctx->clock_probe);
   return grpic_launch_ok();
@@ -602,6 +603,23 @@ extern "C" int grpic_push_deposit(grpic_ctx* ctx, grpic_particles* ptc, const gr
                                               (cudaStream_t)stream);
   grpic_count_launches(1);
   return rc;
+}
+
+// First-order shape with the Vay pusher through the tuned kernel (grpic_push_deposit_variant(1, 1));
+// GRPIC_ERR_ARG when the arrays do not allow the bulk-TMA tiles (the caller then takes the general kernel).
+int grpic_push_deposit_cic_vay(grpic_ctx* ctx, grpic_particles* ptc, const grpic_fields* fields, grpic_current* flux,
+                               double dt, uint32_t* status, cudaStream_t st) {
+  if (!ctx || !ptc_args_ok(ptc) || !grid_args_ok(fields, flux) || !(dt > 0.0) || !tma_aligned(ptc) ||
+      ptc->n > 0xFFFFFFF0LL)
+    return GRPIC_ERR_ARG;
+  if (ptc->n == 0) return GRPIC_OK;
+  const bool tab = ctx->g.dxi <= kSmallStep && ctx->g.dth <= kSmallStep && 2.0 * dt <= kSmallStep * exp(ctx->g.xi_in);
+  grpic_count_launches(1);
+  if (ctx->p.geo_iters != 3)
+    return launch_push_deposit<GRPIC_PD_MA, false, 0, false, true>(ctx, *ptc, *ptc, nullptr, *fields, *flux, dt, status, st);
+  if (!tab)
+    return launch_push_deposit<GRPIC_PD_MA, false, 3, false, true>(ctx, *ptc, *ptc, nullptr, *fields, *flux, dt, status, st);
+  return launch_push_deposit<GRPIC_PD_MA, false, 3, true, true>(ctx, *ptc, *ptc, nullptr, *fields, *flux, dt, status, st);
 }
 
 extern "C" int grpic_push_deposit_compact(grpic_ctx* ctx, const grpic_particles* in, grpic_particles* out,

@@ -191,32 +191,37 @@ __device__ __forceinline__ void boris(const GridDev& g, const Pos& p, double alp
 // e_(3) = d_phi/sqrt(gamma_phiphi); FIDO proper time alpha*dt.  D, B contravariant, u covariant.
 __device__ __forceinline__ void vay(const GridDev& g, const Pos& p, double alpha, double sgn, double dt,
                                     const double D[3], const double B[3], double& ur, double& ut, double& up) {
+  // square roots and quotients through the MUFU-seeded rsqrt_nr / rcp_nr (no division, no sqrt call)
   const double s2 = p.s * p.s;
   const double g_rp = -g.a * s2 * p.zp1, g_pp = s2 * fma(g.a2 * s2, p.zp1, p.rho2);
   const double gu_rr = fma(p.r2a2, p.R, -p.beta);
-  const double sgrr = sqrt(gu_rr), sth = sqrt(p.rho2), sph = sqrt(g_pp);
-  const double k = g_rp / g_pp;
-  const double uh0 = sgrr * (ur - k * up), uh1 = ut / sth, uh2 = up / sph;
-  const double E0 = D[0] / sgrr, E1 = sth * D[1], E2 = (g_rp * D[0] + g_pp * D[2]) / sph;
-  const double B0 = B[0] / sgrr, B1 = sth * B[1], B2 = (g_rp * B[0] + g_pp * B[2]) / sph;
+  const double isgrr = rsqrt_nr(gu_rr), isth = rsqrt_nr(p.rho2), isph = rsqrt_nr(g_pp);
+  const double sgrr = gu_rr * isgrr, sth = p.rho2 * isth, sph = g_pp * isph;
+  const double k = g_rp * (isph * isph);
+  const double uh0 = sgrr * fma(-k, up, ur), uh1 = ut * isth, uh2 = up * isph;
+  const double E0 = D[0] * isgrr, E1 = sth * D[1], E2 = fma(g_rp, D[0], g_pp * D[2]) * isph;
+  const double B0 = B[0] * isgrr, B1 = sth * B[1], B2 = fma(g_rp, B[0], g_pp * B[2]) * isph;
   const double h = sgn * alpha * dt;
-  const double iG0 = 1.0 / sqrt(1.0 + uh0 * uh0 + uh1 * uh1 + uh2 * uh2);
+  const double iG0 = rsqrt_nr(fma(uh0, uh0, fma(uh1, uh1, fma(uh2, uh2, 1.0))));
   const double v0 = uh0 * iG0, v1 = uh1 * iG0, v2 = uh2 * iG0;
-  const double p0 = uh0 + h * (E0 + 0.5 * (v1 * B2 - v2 * B1));
-  const double p1 = uh1 + h * (E1 + 0.5 * (v2 * B0 - v0 * B2));
-  const double p2 = uh2 + h * (E2 + 0.5 * (v0 * B1 - v1 * B0));
-  const double t0 = 0.5 * h * B0, t1 = 0.5 * h * B1, t2 = 0.5 * h * B2;
-  const double tau2 = t0 * t0 + t1 * t1 + t2 * t2;
-  const double ustar = p0 * t0 + p1 * t1 + p2 * t2;
-  const double sigma = 1.0 + p0 * p0 + p1 * p1 + p2 * p2 - tau2;
-  const double G1 = sqrt(0.5 * (sigma + sqrt(sigma * sigma + 4.0 * (tau2 + ustar * ustar))));
-  const double w0 = t0 / G1, w1 = t1 / G1, w2 = t2 / G1;
-  const double udt = p0 * w0 + p1 * w1 + p2 * w2;
-  const double sc = 1.0 / (1.0 + w0 * w0 + w1 * w1 + w2 * w2);
-  const double n0 = sc * (p0 + udt * w0 + (p1 * w2 - p2 * w1));
-  const double n1 = sc * (p1 + udt * w1 + (p2 * w0 - p0 * w2));
-  const double n2 = sc * (p2 + udt * w2 + (p0 * w1 - p1 * w0));
-  ur = n0 / sgrr + n2 * g_rp / sph;
+  const double p0 = fma(h, fma(0.5, v1 * B2 - v2 * B1, E0), uh0);
+  const double p1 = fma(h, fma(0.5, v2 * B0 - v0 * B2, E1), uh1);
+  const double p2 = fma(h, fma(0.5, v0 * B1 - v1 * B0, E2), uh2);
+  const double hh = 0.5 * h;
+  const double t0 = hh * B0, t1 = hh * B1, t2 = hh * B2;
+  const double tau2 = fma(t0, t0, fma(t1, t1, t2 * t2));
+  const double ustar = fma(p0, t0, fma(p1, t1, p2 * t2));
+  const double sigma = fma(p0, p0, fma(p1, p1, fma(p2, p2, 1.0))) - tau2;
+  const double disc = fma(sigma, sigma, 4.0 * fma(ustar, ustar, tau2));     // > 0: sigma >= 1 when tau = 0
+  const double G12 = 0.5 * fma(disc, rsqrt_nr(disc), sigma);                // gamma_new^2
+  const double iG1 = rsqrt_nr(G12);
+  const double w0 = t0 * iG1, w1 = t1 * iG1, w2 = t2 * iG1;
+  const double udt = fma(p0, w0, fma(p1, w1, p2 * w2));
+  const double sc = rcp_nr(fma(w0, w0, fma(w1, w1, fma(w2, w2, 1.0))));
+  const double n0 = sc * (fma(udt, w0, p0) + (p1 * w2 - p2 * w1));
+  const double n1 = sc * (fma(udt, w1, p1) + (p2 * w0 - p0 * w2));
+  const double n2 = sc * (fma(udt, w2, p2) + (p0 * w1 - p1 * w0));
+  ur = fma(n0, isgrr, n2 * g_rp * isph);
   ut = sth * n1;
   up = sph * n2;
 }

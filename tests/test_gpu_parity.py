@@ -549,6 +549,43 @@ def test_push_deposit_variants_parity(G, O, order, pusher, nr, nth, n):
         assert np.max(np.abs(refb["u1"] - ref["u1"])) > 0
 
 
+def test_cic_vay_tuned_and_general_kernels_agree(G, O):
+    """grpic_push_deposit_variant(1, 1) runs the tuned kernel (bulk-TMA tiles, 16-byte aligned particle
+    arrays) and falls back to the general kernel for arrays off that grid: both against the oracle with
+    the Vay option, and against each other."""
+    p = inputs.grid_params(96, 80, 0.99, ng=3)
+    dt = inputs.courant_dt(p)
+    fields = inputs.analytic_fields(p, "wald")
+    n = 50001
+    ptc = inputs.make_particles(p, n, 43, "crowded", ("loguniform", 0.1, 1e3))
+    with O.pusher(1):
+        ref, Fref = oracle_push_deposit(O, p, fields, ptc, dt)
+    ctx = G.Context(p, n)
+    f_t = [ctx.to_device(f) for f in fields]
+    got = []
+    for shift in (0, 1):
+        P = G.Particles(n + shift)
+        if shift:          # views that start one element into their allocations: 8 / 4 bytes off the 16-byte grid
+            P.t = {k: v[1:] for k, v in P.t.items()}
+            P.n = n
+        P.upload(ptc)
+        assert (P.t["x1"].data_ptr() % 16 != 0) == bool(shift)
+        F_t = ctx.zeros(3)
+        ctx.status.zero_()
+        ctx.push_deposit_variant(P, f_t, F_t, dt, shape_order=1, pusher=1)
+        torch.cuda.synchronize()
+        assert int(ctx.status.item()) == 0
+        out = P.to_numpy()
+        with O.pusher(1):
+            check_push(p, ptc, ref, out, O, fields, dt)
+        for c in range(3):
+            assert grid_err(Fref[c], ctx.to_host(F_t[c])) <= 1e-11, c
+        got.append(out)
+    for k in ("x1", "x2", "x3", "u1", "u2", "u3"):
+        assert np.max(np.abs(got[0][k] - got[1][k]) / (np.abs(got[1][k]) + 1e-300)) < 1e-11, k
+    assert np.array_equal(got[0]["cell"], got[1]["cell"]) and np.array_equal(got[0]["flag"], got[1]["flag"])
+
+
 def test_vacuum_wald_relaxation(G, O):
     """Section 3.2 of the paper (Fig.6): the a = 0 Wald field (Eq.25) placed in an
     a = 0.998 Kerr metric evolves, through damped oscillations, to a steady state with H_phi -> 0
