@@ -199,9 +199,6 @@ radix_hist_kernel(const uint32_t* keys, const uint32_t* cell, const uint32_t* fl
 #ifndef GRPIC_SCATTER_MINB
 #define GRPIC_SCATTER_MINB 4
 #endif
-#ifndef GRPIC_SCATTER_BALLOT_GROUPS
-#define GRPIC_SCATTER_BALLOT_GROUPS 0
-#endif
 template <bool FIRST>
 __global__ void __launch_bounds__(kThreads, GRPIC_SCATTER_MINB)
 radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint32_t* cell,
@@ -249,22 +246,11 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
   uint32_t rank_q[kGroups];
 #pragma unroll
   for (int q = 0; q < kGroups; ++q) {
-    // MATCH.ANY executes on the ADU pipe at about one per 6 cycles per SM: 25 M of them are 0.5 ms per
-    // pass at 1e8 keys, which is what a pass took (profiles/r02_late_experiments.md).  The last
-    // GRPIC_SCATTER_BALLOT_GROUPS groups of every thread form the same peer mask on the ALUs instead,
-    // one ballot per digit bit, so that both units work.
-    uint32_t peers;
-    if (q < kGroups - GRPIC_SCATTER_BALLOT_GROUPS) {
-      peers = __match_any_sync(0xffffffffu, dig[q]);
-    } else {
-      peers = 0xffffffffu;
-#pragma unroll
-      for (int b = 0; b < 9; ++b) {                    // bit 8 = the sentinel of lanes beyond n
-        const uint32_t bit = (dig[q] >> b) & 1u;
-        const uint32_t bal = __ballot_sync(0xffffffffu, bit != 0u);
-        peers &= ~(bal ^ (0u - bit));
-      }
-    }
+    // (MATCH.ANY executes on the ADU pipe at about one per 6 cycles per SM: 25 M of them are 0.5 ms per
+    // pass at 1e8 keys, which is what a pass takes.  Forming the peer mask of some of the eight groups on
+    // the ALUs instead -- one ballot per digit bit -- was measured: steady-state sort 5.06 / 5.09 / 5.16 /
+    // 5.22 / 5.26 ms for 0 / 2 / 3 / 4 / 5 groups by ballot; profiles/r02_late_experiments.md)
+    const uint32_t peers = __match_any_sync(0xffffffffu, dig[q]);
     const bool valid = dig[q] < kRadix;
     const uint32_t before = valid ? whist[w][dig[q]] : 0u;
     __syncwarp();
