@@ -154,6 +154,9 @@ def parse(argv=None):
     ap.add_argument("--variant", default="cic-boris", choices=["cic-boris", "cic-vay", "spline3-boris", "spline3-vay"],
                     help="particle shape and momentum update (SURVEY.md 8(f) next-2 / next-3): the default is the "
                          "tuned first-order / generalised-Boris kernel; the others go through grpic_push_deposit_variant")
+    ap.add_argument("--pair-production", action="store_true",
+                    help="after the timed loop (outside it), time grpic_pair_production (SURVEY.md 8(f) next-1: "
+                         "photon emission + pair creation) on the sorted particle state; reported as kernels.pair_production")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -539,6 +542,36 @@ def run_ours(args):
         ms = phases["finalize"]["ms_per_call"]
         kernels["finalize"] = {"ms": ms, "bound": "hbm", "achieved": fb / (ms * 1e-3), "peak": hbm_peak,
                                "unit": "GB/s", "frac": fb / (ms * 1e-3) / hbm_peak}
+
+    # ---- pair production (next-1), outside the timed loop: after a cell sort the removed particles sit
+    # behind the live ones, their slots take the created photons / positrons
+    if args.pair_production and rank == 0:
+        cur_p, alt_p = state
+        ctx.sort(cur_p, alt_p)
+        live = int((alt_p.t["flag"] & 2 == 0).sum().item())
+        n_new = torch.zeros(1, dtype=torch.int64, device="cuda")
+        reps, ts, counts, m = 5, [], [], live
+        for q in range(reps):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(stream)
+            # leptons above gamma = 9.9e4 (0.07 % of the log-uniform momenta) emit a photon of energy 5e4;
+            # a photon converts with probability 0.2 per call: the children fit the slots of the removed particles
+            ctx.pair_production(alt_p, m, n_new, 9.9e4, 5.0e4, 0.2, 12345, q)
+            b.record(stream)
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b))
+            counts.append((m, int(n_new.item())))
+            m = int(n_new.item())
+        # one pass over x1, x2, u1-u3, flag (44 B per particle) + the tile words; per child ~250 B (parent re-read, 2 x 68 B written)
+        pb = (45.0 * np.mean([c[0] for c in counts]) + 250.0 * np.mean([c[1] - c[0] for c in counts])) / 1e9
+        kernels["pair_production"] = {
+            "ms": float(np.mean(ts)), "particles_per_s": float(np.mean([c[0] for c in counts]) / (np.mean(ts) * 1e-3)),
+            "calls": reps, "particles_before_after": counts, "capacity": int(alt_p.n),
+            "bound": "hbm", "achieved": pb / (np.mean(ts) * 1e-3), "peak": hbm_peak, "unit": "GB/s",
+            "frac": pb / (np.mean(ts) * 1e-3) / hbm_peak,
+            "params": {"gamma_thr": 9.9e4, "eps_ph": 5.0e4, "p_convert": 0.2},
+            "status_word": int(ctx.status.item())}
+        state = (alt_p, cur_p)
 
     # ---- end to end: particle state lives in pinned HOST buffers -------------------------
     e2e = None

@@ -73,34 +73,37 @@ __device__ __forceinline__ Event decide(const GridDev& g, const grpic_particles&
   return e;
 }
 
-// pass 1: number of children per 32-particle tile
+// pass 1: number of children per 32-particle tile, and which lanes have one (the second pass reads the
+// particle data of those lanes only: 44 B per particle once instead of twice; 2.53 -> see
+// profiles/r02_late_experiments.md)
 __global__ void __launch_bounds__(256)
 pair_count_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles P,
-                  const __grid_constant__ grpic_pair_params pp, uint32_t* counts) {
+                  const __grid_constant__ grpic_pair_params pp, uint32_t* counts, uint32_t* masks) {
   const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
   bool child = false;
   if (k < P.n) child = decide(g, P, k, pp).child_scale != 0.0;
   const uint32_t b = __ballot_sync(0xffffffffu, child);
-  if ((threadIdx.x & 31) == 0 && k < P.n) counts[k >> 5] = __popc(b);
+  if ((threadIdx.x & 31) == 0 && k < P.n) { counts[k >> 5] = __popc(b); masks[k >> 5] = b; }
 }
 // pass 2: children to n + offsets[tile] + rank, parents updated in place
 __global__ void __launch_bounds__(256)
 pair_apply_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles P,
-                  const __grid_constant__ grpic_pair_params pp, const uint32_t* offsets, uint32_t ntiles,
-                  int64_t capacity, int64_t* n_new, uint32_t* status) {
+                  const __grid_constant__ grpic_pair_params pp, const uint32_t* offsets,
+                  const uint32_t* __restrict__ masks, uint32_t ntiles, int64_t capacity, int64_t* n_new,
+                  uint32_t* status) {
   const int64_t k = (int64_t)blockIdx.x * 256 + threadIdx.x;
   const int lane = threadIdx.x & 31;
-  Event e = {0.0, 1.0, 0u, 0u};
-  if (k < P.n) e = decide(g, P, k, pp);
-  const bool child = e.child_scale != 0.0;
-  const uint32_t b = __ballot_sync(0xffffffffu, child);
   const int64_t tile = k >> 5;
+  if (k >= P.n) return;
+  const uint32_t b = masks[tile];                      // the first pass's decisions (same arithmetic below)
+  const bool child = (b >> lane) & 1u;
   if (k < P.n && tile == (int64_t)ntiles - 1 && lane == 0) {
     const int64_t total = P.n + (int64_t)offsets[tile] + __popc(b);
     *n_new = total < capacity ? total : capacity;
     if (total > capacity && status) atomicOr(status, GRPIC_STATUS_CAPACITY);
   }
   if (!child) return;
+  const Event e = decide(g, P, k, pp);
   const double ur = P.u1[k], ut = P.u2[k], up = P.u3[k];
   const int64_t d = P.n + (int64_t)offsets[tile] + __popc(b & ((1u << lane) - 1u));
   if (d >= capacity) return;      // P5: an event whose child has no room does not happen (parent unchanged)
@@ -128,14 +131,15 @@ extern "C" int grpic_pair_production(grpic_ctx* ctx, grpic_particles* ptc, int64
       !ptc->flag || capacity > 0xFFFFFFF0LL)
     return GRPIC_ERR_ARG;
   const size_t ntiles = (size_t)((n + 31) / 32);
-  const size_t need = (ntiles + ntiles / 2048 + 4096) * sizeof(uint32_t);
+  const size_t need = (2 * ntiles + ntiles / 2048 + 4096) * sizeof(uint32_t);
   if (!ctx->ws || ctx->ws_bytes < need) return GRPIC_ERR_WORKSPACE;
   uint32_t* offsets = (uint32_t*)ctx->ws;
+  uint32_t* masks = offsets + ntiles + ntiles / 2048 + 4096;
   const unsigned grid = (unsigned)((n + 255) / 256);
-  pair_count_kernel<<<grid, 256, 0, st>>>(ctx->g, *ptc, *params, offsets);
+  pair_count_kernel<<<grid, 256, 0, st>>>(ctx->g, *ptc, *params, offsets, masks);
   int rc = grpic_exclusive_scan(offsets, ntiles, offsets + ntiles, st);
   if (rc != GRPIC_OK) return rc;
-  pair_apply_kernel<<<grid, 256, 0, st>>>(ctx->g, *ptc, *params, offsets, (uint32_t)ntiles, capacity, n_new,
+  pair_apply_kernel<<<grid, 256, 0, st>>>(ctx->g, *ptc, *params, offsets, masks, (uint32_t)ntiles, capacity, n_new,
                                           status);
   grpic_count_launches(2);
   return grpic_launch_ok();
