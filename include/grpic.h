@@ -204,7 +204,7 @@ int grpic_step_host(grpic_ctx* ctx, grpic_particles* host_ptc, grpic_fields* fie
  *    ptc->n, ptc->n + 1, ... in the order of their parents.
  * The DEVICE word *n_new receives the new particle count (<= capacity; children beyond capacity
  * are dropped and GRPIC_STATUS_CAPACITY is OR-ed into *status).  ptc->n is NOT changed by the
- * call (the count is only known on the device).  Needs workspace (one word per 32 particles). */
+ * call (the count is only known on the device).  Needs workspace (two words per 32 particles). */
 typedef struct {
   double gamma_thr;   /* threshold FIDO Lorentz factor for emission (paper: 100)       */
   double eps_ph;      /* FIDO energy of an emitted photon (paper: 4.0)                 */
