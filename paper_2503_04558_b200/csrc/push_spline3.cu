@@ -82,8 +82,14 @@ __device__ __forceinline__ void gather_s(const GridDev& g, const double* const (
   }
 }
 
+// resident 128-thread CTAs per SM asked of the compiler (register cap 65536 / (128 MINB)).  The kernel
+// waits on its gather loads (long scoreboard): more warps help more than the spills cost.  Cubic shape at
+// 2e7 particles, ms per push: 1 (128 registers): 5.89, 5 (96, 40 B of stack): 5.07, 6 (80): 5.09, 8 (64): 5.30
+#ifndef GRPIC_S3_MINB
+#define GRPIC_S3_MINB 5
+#endif
 template <int ORDER>
-__global__ void __launch_bounds__(128)
+__global__ void __launch_bounds__(128, GRPIC_S3_MINB)
 push_deposit_general_kernel(const __grid_constant__ GridDev g, const __grid_constant__ grpic_particles ptc,
                             const __grid_constant__ grpic_fields f, const __grid_constant__ grpic_current J,
                             const __grid_constant__ PolyTab pt, double dt, int K, int pusher, uint32_t* status) {
