@@ -44,6 +44,9 @@ constexpr int kBlock = GRPIC_PD_BLOCK;
 //   GRPIC_ABL_NO_BORIS    the Boris step is skipped
 //   GRPIC_ABL_NO_DEPOSIT  no REDs (the deposit arithmetic goes with them)
 //   GRPIC_ABL_K=<n>       n corrector iterations instead of the context's K (0..3)
+//   GRPIC_ABL_SMEM_DEPOSIT  the 8-21 adds of a particle go to a 3 x 128-double tile in SHARED memory
+//                         (atomicAdd on shared doubles) instead of RED.E.ADD.F64 to global memory: the
+//                         arithmetic cost of a CTA-owned J tile without its flush and stray handling
 
 // Charge-conserving deposit of one move (Eq.21-23) on the 3x3-node window anchored at the
 // lower of the old and new cell in each direction: a move of less than one cell touches at
@@ -57,7 +60,7 @@ constexpr int kBlock = GRPIC_PD_BLOCK;
 __device__ __forceinline__ void deposit_local(const PolyTab& pt, const grpic_current& J, uint32_t anchor, uint32_t pitch,
                                               double Q, double vphi, double idt, double fxa, double fya,
                                               double fxb, double fyb, bool oax, bool oay, bool obx,
-                                              bool oby) {
+                                              bool oby, double (*jt)[128] = nullptr) {
   const double gxa = 1.0 - fxa, gya = 1.0 - fya, gxb = 1.0 - fxb, gyb = 1.0 - fyb;
   const double Sa0 = oax ? 0.0 : gxa, Sa1 = oax ? gxa : fxa, Sa2 = oax ? fxa : 0.0;
   const double Sb0 = obx ? 0.0 : gxb, Sb1 = obx ? gxb : fxb, Sb2 = obx ? fxb : 0.0;
@@ -74,6 +77,34 @@ __device__ __forceinline__ void deposit_local(const PolyTab& pt, const grpic_cur
   const double c3 = vphi * pt.v[kR3], c6 = vphi * pt.v[kSIXTH];
   const double U0 = fma(c3, Tb0, c6 * Ta0), U1 = fma(c3, Tb1, c6 * Ta1), U2 = fma(c3, Tb2, c6 * Ta2);
   const double V0 = fma(c3, Ta0, c6 * Tb0), V1 = fma(c3, Ta1, c6 * Tb1), V2 = fma(c3, Ta2, c6 * Tb2);
+#ifdef GRPIC_ABL_SMEM_DEPOSIT
+  {
+    // same slots, same grouping; slot (row r, column c) of the window -> word (anchor + c + 37 r) mod 128
+#define JT(a, r, c) &jt[a][(anchor + (c) + 37u * (r)) & 127u]
+    atomicAdd(JT(0, 0, 0), Ay0 * Px0);          atomicAdd(JT(0, 1, 0), Ay1 * Px0);
+    atomicAdd(JT(1, 0, 0), Ax0 * Py0);          atomicAdd(JT(1, 0, 1), Ax1 * Py0);
+    atomicAdd(JT(2, 0, 0), fma(Sb0, U0, Sa0 * V0));  atomicAdd(JT(2, 0, 1), fma(Sb1, U0, Sa1 * V0));
+    atomicAdd(JT(2, 1, 0), fma(Sb0, U1, Sa0 * V1));  atomicAdd(JT(2, 1, 1), fma(Sb1, U1, Sa1 * V1));
+    if (cx) {
+      atomicAdd(JT(0, 0, 1), Ay0 * Px1);    atomicAdd(JT(0, 1, 1), Ay1 * Px1);
+      atomicAdd(JT(1, 0, 2), Ax2 * Py0);
+      atomicAdd(JT(2, 0, 2), fma(Sb2, U0, Sa2 * V0));    atomicAdd(JT(2, 1, 2), fma(Sb2, U1, Sa2 * V1));
+    }
+    if (cy) {
+      atomicAdd(JT(0, 2, 0), Ay2 * Px0);
+      atomicAdd(JT(1, 1, 0), Ax0 * Py1);  atomicAdd(JT(1, 1, 1), Ax1 * Py1);
+      atomicAdd(JT(2, 2, 0), fma(Sb0, U2, Sa0 * V2));   atomicAdd(JT(2, 2, 1), fma(Sb1, U2, Sa1 * V2));
+      if (cx) {
+        atomicAdd(JT(0, 2, 1), Ay2 * Px1);
+        atomicAdd(JT(1, 1, 2), Ax2 * Py1);
+        atomicAdd(JT(2, 2, 2), fma(Sb2, U2, Sa2 * V2));
+      }
+    }
+#undef JT
+    (void)J; (void)pitch;
+    return;
+  }
+#endif
   double* fr = J.Fr + anchor;
   double* ft = J.Fth + anchor;
   double* fp = J.Fph + anchor;
@@ -200,6 +231,11 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
   // Shared memory is kept below 15872 bytes per CTA on purpose: 8 CTAs then fit the 132 KB carve-out
   // and leave 124 KB of L1 to the gather (the 164 KB carve-out a few bytes more would select: 92 KB).
   __shared__ __align__(16) uint32_t sob[COMPACT ? kWarps : 1][COMPACT ? kPdStages : 1][4];
+#ifdef GRPIC_ABL_SMEM_DEPOSIT
+  __shared__ double jtile[3][128];
+  for (int q = threadIdx.x; q < 3 * 128; q += kBlock) (&jtile[0][0])[q] = 0.0;
+  __syncthreads();
+#endif
   uint32_t tid_x;
   asm volatile("mov.u32 %0, %%tid.x;" : "=r"(tid_x));
   const uint32_t lane = tid_x & 31u;
@@ -476,8 +512,13 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
       const int di = ib - ia, dj = jb - ja;
       if ((uint32_t)(di + 1) <= 2u && (uint32_t)(dj + 1) <= 2u) {
         const int iw = min(ia, ib), jw = min(ja, jb);
+#ifdef GRPIC_ABL_SMEM_DEPOSIT
+        deposit_local(pt, J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - fin, ya - fjn, fxb,
+                      fyb, ia != iw, ja != jw, ib != iw, jb != jw, jtile);
+#else
         deposit_local(pt, J, (uint32_t)g.idx(iw, jw), (uint32_t)g.pitch, q, vph, idt, xa - fin, ya - fjn, fxb,
                       fyb, ia != iw, ja != jw, ib != iw, jb != jw);
+#endif
       } else {
         deposit_far(&g, q, idt, vph, xa, xb, ya, yb, J.Fr, J.Fth, J.Fph, status);
       }
@@ -490,6 +531,10 @@ push_deposit_kernel(const __grid_constant__ GridDev g, const __grid_constant__ g
     tile += wstride;
   }
   }
+#ifdef GRPIC_ABL_SMEM_DEPOSIT
+  __syncthreads();      // the tile's content goes somewhere, so that the adds above are not dead code
+  for (int q = threadIdx.x; q < 3 * 128; q += kBlock) atomicAdd(J.Fr + q, (&jtile[0][0])[q] * 1e-300);
+#endif
   if (probe) {
     unsigned long long t;
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
