@@ -315,7 +315,8 @@ radix_scatter_kernel(const uint32_t* keys_in, const uint32_t* idx_in, const uint
 // load behind the previous store (ten dependent memory round trips per thread; 2.88 ms at 1e8
 // particles against the time noted in profiles/r02_final.md for this form).  (Loads with the
 // L2::64B fetch-size hint were measured: first sort of a random order 23.9 -> 22.9 ms, steady
-// state 5.28 -> 5.36 ms; not kept.)
+// state 5.28 -> 5.36 ms; not kept.  Two / four particles per thread, all loads before the first store:
+// steady-state sort 5.10 -> 5.11 / 5.15 ms; not kept.)
 __global__ void __launch_bounds__(256)
 gather_particles_kernel(grpic_particles in, grpic_particles out, const uint32_t* __restrict__ perm,
                         uint32_t* __restrict__ perm_out) {
