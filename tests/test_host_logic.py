@@ -173,3 +173,22 @@ def test_allreduce_flux_uses_one_collective_for_a_block(monkeypatch):
     calls.clear()
     sharding.allreduce_flux([torch.zeros(4, 8) for _ in range(3)])
     assert calls == [32, 32, 32]
+
+
+def test_bench_variant_option_and_guard_nodes():
+    """bench.py --variant: the cubic-spline shape needs three guard nodes, so the workload of those
+    variants is generated with ng = 3 (array shapes follow), the others with BASELINE's ng = 2; the
+    option is parsed with the tuned kernel as default."""
+    import bench
+    assert bench.parse([]).variant == "cic-boris"
+    for variant, ng in (("cic-vay", 2), ("spline3-boris", 3), ("spline3-vay", 3)):
+        args = bench.parse(["--variant", variant, "--config", "1", "--grid", "24", "--particles", "50"])
+        cfg = bench.workload(args, 0)
+        p = cfg["params"]
+        assert p["ng"] == ng and (p["nr"], p["nth"]) == (24, 24)
+        assert all(f.shape == inputs.grid_shape(p) for f in cfg["fields"])
+        assert len(cfg["particles"]["x1"]) == 50
+        cfg1 = bench.workload(args, 1)            # another rank: same grid, its own particles
+        assert cfg1["params"]["ng"] == ng and not np.array_equal(cfg1["particles"]["x1"], cfg["particles"]["x1"])
+    with pytest.raises(SystemExit):
+        bench.parse(["--variant", "spline5"])
