@@ -663,9 +663,12 @@ def test_continuity_residual_gpu(G, O):
     assert np.max(np.abs(inner)) <= 1e-13 * scale, np.max(np.abs(inner)) / scale
 
 
-@pytest.mark.parametrize("kind,damp", [("wald", 0), ("monopole", 9)])
-def test_field_step_parity(G, O, kind, damp):
-    p = inputs.grid_params(90, 70, 0.9, r_out=30.0, damp_cells=damp, damp_coef=0.7)
+@pytest.mark.parametrize("kind,damp,ng", [("wald", 0, 2), ("monopole", 9, 2), ("wald", 0, 3), ("monopole", 5, 4)])
+def test_field_step_parity(G, O, kind, damp, ng):
+    """Three field steps (predictor + N correctors, axis values, radial guards, ghost rows, damping
+    layer) element by element against the oracle, guard nodes included; ng = 3 is the layout of the
+    cubic-spline runs, ng = 4 exercises the guard loops beyond it."""
+    p = inputs.grid_params(90, 70, 0.9, r_out=30.0, damp_cells=damp, damp_coef=0.7, ng=ng)
     dt = inputs.courant_dt(p)
     rng = np.random.default_rng(3)
     bg = inputs.analytic_fields(p, kind)
