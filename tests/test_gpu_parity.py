@@ -663,6 +663,24 @@ def test_continuity_residual_gpu(G, O):
     assert np.max(np.abs(inner)) <= 1e-13 * scale, np.max(np.abs(inner)) / scale
 
 
+@pytest.mark.parametrize("nr,nth,ng", [(37, 29, 2), (130, 67, 3), (260, 131, 2)])
+def test_fill_guards_bit_exact(G, O, nr, nth, ng):
+    """grpic_fill_guards (axis values, radial guards, theta ghost rows: one launch whose threads compose
+    the three rules) on arrays whose every entry, guards included, is random: bit for bit the oracle's
+    boundary pass (copies and sign flips only), corners of guard columns x ghost rows included."""
+    p = inputs.grid_params(nr, nth, 0.9, ng=ng)
+    rng = np.random.default_rng(nr + ng)
+    f = [rng.standard_normal(inputs.grid_shape(p)) for _ in range(6)]
+    ref = O.apply_bc(p, [x.copy() for x in f])
+    ctx = G.Context(p)
+    f_t = [ctx.to_device(x) for x in f]
+    ctx.fill_guards(f_t)
+    torch.cuda.synchronize()
+    for c in range(6):
+        got = ctx.to_host(f_t[c])
+        assert np.array_equal(got, ref[c]), (c, np.argwhere(got != ref[c])[:5])
+
+
 @pytest.mark.parametrize("kind,damp,ng", [("wald", 0, 2), ("monopole", 9, 2), ("wald", 0, 3), ("monopole", 5, 4)])
 def test_field_step_parity(G, O, kind, damp, ng):
     """Three field steps (predictor + N correctors, axis values, radial guards, ghost rows, damping
