@@ -301,7 +301,7 @@ def test_photon_species_parity(G, O):
     assert grid_err(O.rho(p, alive, ptc["w"]), ctx.to_host(rho)) <= 1e-11
 
 
-@pytest.mark.parametrize("n,cap,step", [(20000, 40000, 3), (777, 800, 0), (0, 16, 1)])
+@pytest.mark.parametrize("n,cap,step", [(20000, 40000, 3), (777, 800, 0), (0, 16, 1), (300007, 450000, 2), (300007, 330000, 5)])
 def test_pair_production_parity(G, O, n, cap, step):
     """grpic_pair_production vs the oracle (Eq.26): who emits / converts, the
     new particle count and the append ORDER bit-exact (same Philox numbers on both sides),
